@@ -1,0 +1,367 @@
+#!/usr/bin/env python
+"""bench.py -- particle-steps/s of the hot path on BASELINE.json's config[1] (default), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+
+One bench "step" = one pass of the whole hot path over one batch of synthetic input
+(SURVEY.md 8(a) rows S0-S7): create + init the ensemble from its Philox init blocks, bind the
+snapshot buffer, integrate all n_steps of the config (one frame every K_snap steps), reduce the
+ensemble moments, destroy.  `value` times that on the device (CUDA events on the launching
+stream, parameters already marshalled); `e2e` times the same pass by wall clock through the
+C ABI from HOST parameter records to HOST results, including a device->host copy of the final
+frame into pinned memory and of the moments.
+
+N > 1 (torchrun): each rank integrates its own shard of a N-times larger ensemble (weak scaling;
+trajectory indices rank*T ... via traj_base), and the only exchange is one all-reduce of the
+per-set raw moment sums (8 doubles per set) over NCCL, inside the timed region.
+
+--impl reference times the CPU oracle (oracle/, plain fp64 C) on a bounded sample of the same
+workload on the host cores: a deliberately slow program, reported as the baseline, not the target.
+"""
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1104_2499_b200 import workloads as W  # noqa: E402
+
+# Algorithmic (necessary) warp-lane instructions per particle-step, frozen in BASELINE.md /
+# DESIGN.md before tuning.
+I_ALG = {0: 29.0, 1: 29.0, 2: 29.0, 3: 45.0, 4: 110.0}
+N_SM, LANES_PER_SM = 148, 128
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return json.load(open(path)), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks sampled DURING the timed region
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    def __init__(self, index=0, period=0.05):
+        self.index, self.period = index, period
+        self.sm, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20,
+                 "hw_thermal_slowdown": 0x40, "hw_power_brake": 0x80, "sync_boost": 0x10,
+                 "app_clocks": 0x2}
+        while not self._stop.is_set():
+            try:
+                self.sm.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+
+    def summary(self):
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(statistics.median(self.sm)), "sm_max_mhz": float(self.max_mhz),
+                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline and --impl reference): the ONLY places bench.py touches oracle/
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(wl, every, n_steps, threads):
+    """Oracle on every `every`-th trajectory of set 0 for the first n_steps steps -> (psteps, seconds)."""
+    from oracle import abm_oracle as orc
+    p = wl.set_params(0)
+    n = max(wl.n_particles // every, 1)
+    x, v, e = orc.init_many(p, wl.seed, n, 0, every)
+    t0 = time.perf_counter()
+    orc.run(p, wl.seed, x, v, e, 0, n_steps, 0, every, threads=threads)
+    dt = time.perf_counter() - t0
+    assert np.isfinite(x).all()
+    return n * n_steps, dt
+
+
+def cpu_baseline(wl, budget_s=6.0):
+    """Oracle as it stands on the host cores: one thread, then the same loop split over all cores."""
+    from oracle import abm_oracle as orc
+    cores = orc.host_threads()
+    every1 = max(wl.n_particles // 2048, 1)
+    ps, dt = oracle_sample(wl, every1, 200, 1)            # calibrate
+    rate1 = ps / dt
+    n1 = int(max(200, min(wl.n_steps, budget_s * rate1 / (wl.n_particles // every1))))
+    ps1, dt1 = oracle_sample(wl, every1, n1, 1)
+    everyN = max(wl.n_particles // (2048 * cores), 1)
+    psN, dtN = oracle_sample(wl, everyN, n1, cores)
+    return {
+        "value": psN / dtN, "unit": "particle-steps/s", "cores": cores, "kind": "oracle",
+        "single_thread_value": ps1 / dt1,
+        "sample": f"{wl.name}: every {everyN}th trajectory ({wl.n_particles // everyN}) x first {n1} "
+                  f"steps on {cores} threads ({psN:.3g} particle-steps in {dtN:.2f} s); single thread: "
+                  f"every {every1}th x {n1} steps in {dt1:.2f} s; fp64, plain C, not tuned",
+    }
+
+
+def run_reference(args, wl):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import abm_oracle as orc
+    cores = orc.host_threads()
+    every = max(wl.n_particles // (2048 * cores), 1)
+    n_steps = 1000
+    for _ in range(args.warmup):
+        oracle_sample(wl, every, 100, cores)
+    tot_ps, tot_t = 0, 0.0
+    for _ in range(args.steps):
+        ps, dt = oracle_sample(wl, every, n_steps, cores)
+        tot_ps += ps
+        tot_t += dt
+    val = tot_ps / tot_t
+    sample = (f"each step = every {every}th trajectory ({wl.n_particles // every}) x first {n_steps} steps "
+              f"of {wl.name} on {cores} host threads")
+    print(json.dumps({
+        "impl": "reference", "metric": "particle-steps/sec", "value": val, "unit": "particle-steps/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": "particle-steps/s", "cores": cores, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": val, "unit": "particle-steps/s", "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args, wl, cfg_id):
+    import torch
+    import torch.distributed as dist
+    from paper_1104_2499_b200 import binding as abm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference "
+                         "for the oracle)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    abm.lib()
+
+    stream = torch.cuda.Stream()
+    sets = [wl.set_params(s) for s in range(wl.n_param_sets)]
+    T = wl.n_trajectories
+    # weak scaling: rank r owns global trajectories [r*T, (r+1)*T); whole sets stay on one rank
+    traj_base = rank * T
+    n_steps, M = wl.n_steps, (wl.moments_every or wl.n_steps)
+    fp64 = sets[0]["precision"] == 1
+    frame_cols = 2
+    frame_item = 8 if fp64 else 4
+    host_frame = torch.empty((T, frame_cols), dtype=torch.float64 if fp64 else torch.float32,
+                             pin_memory=True)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+    launches = {"n": 0}
+    ens_tilt = any(p["A"] != 0.0 for p in sets)
+    step_launches = (2 if ens_tilt else 1) * -(-M // (65536 if ens_tilt else 2**30))
+    # parameter records marshalled once (host side); abm_create copies them to the device
+    params = abm.make_params(sets, stream=stream.cuda_stream, snapshot_every=wl.snapshot_every,
+                             traj_base=traj_base)
+    params_bytes = len(sets) * abm.C.sizeof(abm.abm_params)
+
+    def one_pass(e2e, ev=None):
+        """The whole hot path once.  Returns the moments (host)."""
+        with torch.cuda.stream(stream):
+            ens = abm.Ensemble(params, wl.n_particles, wl.seed, stream=stream)  # S0 (1 kernel)
+            launches["n"] += 1
+            if wl.snapshot_every:
+                ens.bind_snapshot()                                            # S5 (1 kernel)
+                launches["n"] += 1
+            m = None
+            for _ in range(n_steps // M):
+                if ev is not None:
+                    ev[0].record(stream)
+                ens.step(M)                                                    # S1-S5, S7
+                if ev is not None:
+                    ev[1].record(stream)
+                launches["n"] += step_launches
+                if world > 1:
+                    sums = torch.from_numpy(ens.moment_sums()).cuda()          # S6 (2 kernels)
+                    dist.all_reduce(sums)
+                    m = abm.abm_moments_from_sums(sums.cpu().numpy(), ens.step_count)
+                else:
+                    m = ens.moments()                                          # S6 (2 kernels)
+                launches["n"] += 2
+            if e2e:
+                abm.abm_snapshot_host(ens.ctx, host_frame.numpy(), frame_cols * frame_item)
+                launches["n"] += 1
+            ens.close()
+        return m
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        one_pass(False)
+        one_pass(True)
+    barrier()
+
+    # ---- device-timed arm -------------------------------------------------------------------
+    ev_pass = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+               for _ in range(args.steps)]
+    ev_kern = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+               for _ in range(args.steps)]
+    launches["n"] = 0
+    barrier()
+    wall0 = time.perf_counter()
+    with ClockSampler(local_rank) as clk:
+        for i in range(args.steps):
+            flush.fill_(i & 0xff)                       # L2 flush between timed iterations
+            torch.cuda.synchronize()
+            ev_pass[i][0].record(stream)
+            m = one_pass(False, ev_kern[i] if n_steps == M else None)
+            ev_pass[i][1].record(stream)
+        barrier()
+    wall = time.perf_counter() - wall0
+    gpu_launches = launches["n"]
+    t_pass_ms = [a.elapsed_time(b) for a, b in ev_pass]
+    t_dev = sum(t_pass_ms) * 1e-3
+    t_kern_ms = [a.elapsed_time(b) for a, b in ev_kern] if n_steps == M else None
+
+    # ---- end-to-end arm (host params -> host frame + moments), wall clock ---------------------
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        m_e2e = one_pass(True)
+    barrier()
+    t_e2e = time.perf_counter() - t0
+
+    tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    t_dev, t_e2e = float(tt[0]), float(tt[1])
+
+    psteps_job = wl.particle_steps * world * args.steps
+    value = psteps_job / t_dev
+    peaks, peak_src = load_peaks()
+    f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
+    clocks = clk.summary()
+
+    out = {
+        "metric": "particle-steps/sec", "value": value, "unit": "particle-steps/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None,   # the paper states no throughput for this path
+        "dtype": "f64" if fp64 else "f32", "data": "synthetic",
+        "config": {"workload": wl.name, "baseline_config": cfg_id, "trajectories_per_gpu": T,
+                   "param_sets": wl.n_param_sets, "sim_steps": n_steps,
+                   "snapshot_every": wl.snapshot_every, "moments_every": M,
+                   "integrator": "heun" if sets[0]["integrator"] else "euler-maruyama",
+                   "l2": "flushed between timed iterations (256 MiB fill)",
+                   "pass": "create+init, bind frame, integrate, moments, destroy"},
+        "e2e": {"value": psteps_job / t_e2e, "unit": "particle-steps/s",
+                "h2d_bytes_per_step": int(params_bytes),
+                "d2h_bytes_per_step": int(host_frame.numel() * host_frame.element_size()
+                                          + 80 * len(sets) * (n_steps // M)),
+                "timer": "wall clock, host parameter records -> pinned host frame + moments"},
+        "gpu_launches": gpu_launches,
+        "clocks": clocks,
+        "wall_s_timed_region": wall,
+    }
+    if t_kern_ms:
+        t_k = statistics.mean(t_kern_ms) * 1e-3
+        lane_instr = I_ALG[cfg_id] * wl.particle_steps
+        peak = N_SM * LANES_PER_SM * f_max
+        achieved = lane_instr / t_k
+        sm_mhz = clocks.get("sm_mhz") or (f_max / 1e6)
+        out["roofline"] = {
+            "bound": "alu", "kernel": "abm::step_kernel", "achieved": achieved / 1e12,
+            "peak": peak / 1e12, "unit": "Tinstr/s (warp-lane instructions)",
+            "frac": achieved / peak,
+            "frac_at_sustained_clock": achieved / (N_SM * LANES_PER_SM * sm_mhz * 1e6),
+            "i_alg_per_particle_step": I_ALG[cfg_id],
+            "particle_steps_per_launch": wl.particle_steps,
+            "kernel_ms": 1e3 * t_k, "kernel_share_of_pass": sum(t_kern_ms) / sum(t_pass_ms),
+            "peak_source": f"148 SMs x 128 lanes x sm_max_mhz {f_max / 1e6:.0f} MHz, {peak_src}",
+            "traffic": None,
+            "hbm_algorithmic_bytes_per_launch": int(T * (24 + 8 * (n_steps // wl.snapshot_every
+                                                                   if wl.snapshot_every else 0))),
+        }
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(wl)
+        m0 = m[0]
+        out["result"] = {"step": int(m0["step"]), "mean_v": float(m0["mean_v"]),
+                         "var_x": float(m0["var_x"]), "mean_e": float(m0["mean_e"])}
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sim-steps", type=int, default=0, help="override the config's step count")
+    args = ap.parse_args()
+    wl = W.CONFIGS[args.config]()
+    if args.sim_steps:
+        wl.n_steps = args.sim_steps
+        if wl.moments_every:
+            wl.moments_every = min(wl.moments_every, wl.n_steps)
+    if args.impl == "reference":
+        run_reference(args, wl)
+    else:
+        run_ours(args, wl, args.config)
+
+
+if __name__ == "__main__":
+    main()

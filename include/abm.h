@@ -1,0 +1,160 @@
+/*
+ * abm.h -- C ABI of the B200-native hot path of arXiv 1104.2499 (M. Zabicki, "OpenCL/OpenGL
+ * approach for studying active Brownian motion"): integration of a large ensemble of
+ * independent energy-depot active-Brownian trajectories on a ratchet potential, device-side
+ * snapshots in place of the paper's shared OpenGL vertex buffer, and ensemble moments.
+ *
+ * Citations are PAPER.md line numbers (+ section / equation / figure) or BASELINE.json.
+ *
+ * The model (one trajectory = the paper's "work item"):
+ *     dx/dt = v                                                        (implied by Eqs. 2-3)
+ *     dv/dt = F0 + d e v - gamma0 v - U'(x) + A cos(omega t) + sqrt(2D) xi(t)
+ *                                                (Eq. 2; tilt: BASELINE.json)
+ *     de/dt = q - c e - d e v^2                                        (Eq. 1)
+ *     U(x)  = A1 sin(th) + A2 sin(2 th) + const,  th = 2 pi (x + phi) / L  (Eq. 3)
+ * The paper's own potential of height h is L = 1, phi = 0.1903, A1 = -0.453 h, A2 = -0.11325 h.
+ *
+ * The loop each trajectory runs is the paper's pseudo kernel (Fig. 1): read the
+ * parameters, for every step draw a uniform pair, Box-Muller it, compute the new velocity and
+ * energy, and write the state back at the end so the next launch continues.  The generator is
+ * counter-based Philox4x32-10 keyed by (seed, trajectory, step) instead of the paper's
+ * xorshift (BASELINE.json north_star (b)); the exact stream is documented in
+ * DESIGN.md ("Random stream") and is the same one the CPU oracle consumes.
+ *
+ * Conventions
+ *   - All functions are extern "C", take plain pointers and sizes, and never throw.
+ *   - Return value: ABM_OK (0) or a negative abm_status; *out arguments are untouched on error.
+ *   - Pointers are HOST pointers unless the parameter is named dev_* (DEVICE pointer, valid on
+ *     the device that was current at abm_create).
+ *   - Trajectory index:  i = traj_base + set * traj_set_stride + r,   r < n_particles,
+ *     set < n_param_sets; with the defaults (traj_base = 0, traj_set_stride = 0 meaning
+ *     n_particles) this is i = set * n_particles + r.  The random stream, and therefore the
+ *     whole trajectory, depends only on (seed, i, parameters): shards of one ensemble on
+ *     several GPUs use traj_base / traj_set_stride to address disjoint index ranges.
+ *   - In device buffers trajectories are stored in local order  k = set * n_particles + r.
+ *   - The library owns the state and its scratch; `params` may be freed after abm_create; the
+ *     snapshot buffer and all `out` arrays are caller-owned.
+ *   - One context is not thread-safe; distinct contexts are independent.  All work of a context
+ *     is enqueued on params[0].stream in call order; only abm_moments, abm_moment_sums,
+ *     abm_snapshot_host and abm_destroy wait for it.
+ *   - There is no CPU fallback: without a CUDA device abm_create returns ABM_ECUDA.
+ */
+#ifndef ABM_H
+#define ABM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum abm_status {
+  ABM_OK = 0,
+  ABM_EINVAL = -1, /* null pointer, struct_size mismatch, zero counts, run-control fields that
+                      differ between parameter sets, unsupported stride, misaligned pointer,
+                      non-finite or non-positive dt / L / gamma0 (when init_v = 1)             */
+  ABM_ENOMEM = -2, /* device or host allocation failed                                        */
+  ABM_ECUDA = -3,  /* CUDA error (sticky: reported by this and every later call)              */
+  ABM_ESTATE = -4  /* null or destroyed context                                               */
+} abm_status;
+
+enum { ABM_FP32 = 0, ABM_FP64 = 1 };               /* abm_params.precision  */
+enum { ABM_EULER_MARUYAMA = 0, ABM_HEUN = 1 };     /* abm_params.integrator */
+enum { ABM_INIT_V_CONST = 0, ABM_INIT_V_THERMAL = 1 }; /* abm_params.init_v */
+
+typedef struct abm_ctx abm_ctx; /* opaque, owned by the library */
+
+/* One record per parameter set (the paper's per-work-item parameter record).
+ * POD; copied at abm_create.  "Run-control" fields (marked RC) must be equal in all sets. */
+typedef struct abm_params {
+  uint32_t struct_size;    /* RC  = sizeof(abm_params); ABI guard                              */
+  uint32_t precision;      /* RC  ABM_FP32 | ABM_FP64 (SP main path, DP optional)  */
+  uint32_t integrator;     /* RC  ABM_EULER_MARUYAMA | ABM_HEUN                                */
+  uint32_t init_v;         /* RC  v(0) = v0, or v(0) ~ N(0, D/gamma0) from the init block      */
+  uint32_t snapshot_every; /* RC  K: abm_step rewrites the bound snapshot buffer after every
+                                  global step count that is a multiple of K; 0 = never         */
+  uint32_t reserved0;
+  double dt;               /* RC  time step                                                    */
+  double gamma0, q, c, d, D; /*   Eqs. 1-2                                                     */
+  double F0;               /*     constant load force, +F0 as printed in Eq. 2   */
+  double A, omega;         /*     tilt A cos(omega n dt), n = global 0-based step index;
+                                  omega is RC (one tilt table per launch), A is per set        */
+  double L, A1, A2, phi;   /*     potential (see top of file)                                  */
+  double v0, e0;           /*     constant initial values (x(0) ~ U[0, L) always)              */
+  uint64_t traj_base;      /* RC  first global trajectory index of this context                */
+  uint64_t traj_set_stride;/* RC  index distance between consecutive sets; 0 = n_particles     */
+  void* stream;            /* RC  cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream);
+                                  NULL = the legacy default stream                             */
+} abm_params;
+
+/* Ensemble moments of one parameter set over its n_particles realisations ("results are
+ * averaged"), population normalisation 1/N, at global step `step`.
+ * dx = x - x(0), with x(0) recomputed from the trajectory's init block. */
+typedef struct abm_moment {
+  uint64_t n, step;
+  double mean_x, var_x, mean_v, var_v, mean_e, mean_dx, mean_dx2, mean_x2;
+} abm_moment; /* 80 bytes */
+
+/* Raw fp64 sums behind abm_moment, for combining shards (one record per set):
+ * s = { N, sum x, sum x^2, sum v, sum v^2, sum e, sum dx, sum dx^2 },
+ * with x and v taken relative to the set's first trajectory's initial values is NOT done:
+ * the sums are plain; they are accumulated in fp64 in a fixed order (run-to-run reproducible). */
+#define ABM_N_SUMS 8
+
+/* Create a context for n_param_sets parameter sets x n_particles trajectories each and
+ * initialise every trajectory from its Philox init block (S0): x(0) = L u, v(0), e(0) = e0.
+ * Reads params[0 .. n_param_sets) (HOST).  Enqueues on params[0].stream; does not wait. */
+int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_sets,
+               uint64_t seed, abm_ctx** out);
+
+/* Advance every trajectory by n_steps steps (S1-S5, S7; Fig. 1's loop), in one or a
+ * few kernel launches with the state in registers in between.  Asynchronous.
+ * abm_step(a); abm_step(b) is bit-identical to abm_step(a + b). n_steps = 0 is a no-op. */
+int abm_step(abm_ctx* ctx, uint64_t n_steps);
+
+/* Snapshot sink -- the headless replacement of the shared OpenGL vertex buffer.
+ * dev_ptr != NULL: write the current state of all trajectories to dev_ptr now, and bind it as
+ * the buffer that abm_step overwrites after every K-th step (K = snapshot_every; one frame,
+ * overwritten).  dev_ptr == NULL: unbind.  stride_bytes = distance between trajectories:
+ *   fp32:  8 -> float2 (x, v)        16 -> float4 (x, v, e, 1.0f)  (homogeneous vertex, :162)
+ *   fp64: 16 -> double2 (x, v)       32 -> double4 (x, v, e, 1.0)
+ * dev_ptr must be aligned to stride_bytes and hold n_particles * n_param_sets * stride_bytes. */
+int abm_snapshot(abm_ctx* ctx, void* dev_ptr, size_t stride_bytes);
+
+/* Same frame, copied to HOST memory (the paper's non-shared path); waits. */
+int abm_snapshot_host(abm_ctx* ctx, void* host_ptr, size_t stride_bytes);
+
+/* Ensemble moments of every set at the current step (S6): warp-shuffle + block + fixed-order
+ * grid reduction in fp64 on the device, then a copy to out[0 .. n_param_sets) (HOST); waits. */
+int abm_moments(abm_ctx* ctx, abm_moment* out);
+
+/* The raw sums (HOST, out[n_param_sets][ABM_N_SUMS]) and the pure host-side finalisation used
+ * after summing shards: out_moments[s] from sums[s]. */
+int abm_moment_sums(abm_ctx* ctx, double* out);
+int abm_moments_from_sums(const double* sums, uint32_t n_param_sets, uint64_t step,
+                          abm_moment* out_moments);
+
+/* Global step count reached so far. */
+int abm_get_step(const abm_ctx* ctx, uint64_t* out_step);
+
+/* Wait for the context's stream and free everything the library owns. */
+int abm_destroy(abm_ctx* ctx);
+
+/* Diagnostics of the random stream (tests: "bit-exact for the RNG integer stream").
+ * dev_out[(k * n_blocks + j) * 4 + w] = word w of Philox block block_first + j of trajectory
+ * traj_first + k -- produced by the same device function the step kernels call.
+ * stream: cudaStream_t or NULL.  Asynchronous. */
+int abm_philox_blocks(uint64_t seed, uint64_t traj_first, uint64_t n_traj, uint64_t block_first,
+                      uint64_t n_blocks, uint32_t* dev_out, void* stream);
+
+/* Static, non-owning description of a status code. */
+const char* abm_strerror(int status);
+
+/* Version of this ABI (bumped when abm_params or a signature changes). */
+uint32_t abm_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ABM_H */

@@ -1,0 +1,250 @@
+"""Thin ctypes binding of the C ABI in include/abm.h -- same names, argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind `libabm_b200.so`; this module never
+computes anything itself and has no fallback: if the library is missing or a call fails it raises.
+PyTorch is used by callers for device memory (snapshot buffers) and streams; this module only
+passes raw pointers / stream handles through.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libabm_b200.so")
+
+ABM_OK, ABM_EINVAL, ABM_ENOMEM, ABM_ECUDA, ABM_ESTATE = 0, -1, -2, -3, -4
+ABM_FP32, ABM_FP64 = 0, 1
+ABM_EULER_MARUYAMA, ABM_HEUN = 0, 1
+ABM_N_SUMS = 8
+
+
+class abm_params(C.Structure):
+    """Mirror of `abm_params` (include/abm.h)."""
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("precision", C.c_uint32), ("integrator", C.c_uint32),
+        ("init_v", C.c_uint32), ("snapshot_every", C.c_uint32), ("reserved0", C.c_uint32),
+        ("dt", C.c_double), ("gamma0", C.c_double), ("q", C.c_double), ("c", C.c_double),
+        ("d", C.c_double), ("D", C.c_double), ("F0", C.c_double), ("A", C.c_double),
+        ("omega", C.c_double), ("L", C.c_double), ("A1", C.c_double), ("A2", C.c_double),
+        ("phi", C.c_double), ("v0", C.c_double), ("e0", C.c_double),
+        ("traj_base", C.c_uint64), ("traj_set_stride", C.c_uint64), ("stream", C.c_void_p),
+    ]
+
+
+class abm_moment(C.Structure):
+    """Mirror of `abm_moment` (include/abm.h), 80 bytes."""
+    _fields_ = [("n", C.c_uint64), ("step", C.c_uint64), ("mean_x", C.c_double),
+                ("var_x", C.c_double), ("mean_v", C.c_double), ("var_v", C.c_double),
+                ("mean_e", C.c_double), ("mean_dx", C.c_double), ("mean_dx2", C.c_double),
+                ("mean_x2", C.c_double)]
+
+
+MOMENT_DTYPE = np.dtype([("n", "<u8"), ("step", "<u8"), ("mean_x", "<f8"), ("var_x", "<f8"),
+                         ("mean_v", "<f8"), ("var_v", "<f8"), ("mean_e", "<f8"),
+                         ("mean_dx", "<f8"), ("mean_dx2", "<f8"), ("mean_x2", "<f8")])
+
+EXPORTS = ["abm_create", "abm_step", "abm_snapshot", "abm_snapshot_host", "abm_moments",
+           "abm_moment_sums", "abm_moments_from_sums", "abm_get_step", "abm_destroy",
+           "abm_philox_blocks", "abm_strerror", "abm_abi_version"]
+
+_lib = None
+
+
+class AbmError(RuntimeError):
+    def __init__(self, fn, status):
+        self.status = status
+        msg = lib().abm_strerror(status).decode() if _lib is not None else str(status)
+        super().__init__(f"{fn} failed: {status} ({msg})")
+
+
+def lib():
+    """Load libabm_b200.so (built by paper_1104_2499_b200/build.py).  No fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_1104_2499_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, u64, u32 = C.c_void_p, C.c_uint64, C.c_uint32
+        L.abm_create.argtypes = [C.POINTER(abm_params), u64, u32, u64, C.POINTER(vp)]
+        L.abm_step.argtypes = [vp, u64]
+        L.abm_snapshot.argtypes = [vp, vp, C.c_size_t]
+        L.abm_snapshot_host.argtypes = [vp, vp, C.c_size_t]
+        L.abm_moments.argtypes = [vp, vp]
+        L.abm_moment_sums.argtypes = [vp, vp]
+        L.abm_moments_from_sums.argtypes = [vp, u32, u64, vp]
+        L.abm_get_step.argtypes = [vp, C.POINTER(u64)]
+        L.abm_destroy.argtypes = [vp]
+        L.abm_philox_blocks.argtypes = [u64, u64, u64, u64, u64, vp, vp]
+        for n in EXPORTS[:-2]:
+            getattr(L, n).restype = C.c_int
+        L.abm_strerror.argtypes = [C.c_int]
+        L.abm_strerror.restype = C.c_char_p
+        L.abm_abi_version.argtypes = []
+        L.abm_abi_version.restype = C.c_uint32
+        _lib = L
+    return _lib
+
+
+_PARAM_KEYS = ["precision", "integrator", "init_v", "snapshot_every", "dt", "gamma0", "q", "c", "d",
+               "D", "F0", "A", "omega", "L", "A1", "A2", "phi", "v0", "e0", "traj_base",
+               "traj_set_stride"]
+
+
+def make_params(param_sets, stream=0, **common):
+    """list of dicts (one per parameter set) -> ctypes array of abm_params."""
+    arr = (abm_params * len(param_sets))()
+    for s, d in enumerate(param_sets):
+        p = arr[s]
+        p.struct_size = C.sizeof(abm_params)
+        for k in _PARAM_KEYS:
+            if k in common:
+                setattr(p, k, common[k])
+            elif k in d:
+                setattr(p, k, d[k])
+        p.stream = stream or None
+    return arr
+
+
+def _check(fn, status):
+    if status != ABM_OK:
+        raise AbmError(fn, status)
+
+
+# ---- the calls, one-to-one -------------------------------------------------------------------
+
+def abm_create(params, n_particles, n_param_sets, seed):
+    h = C.c_void_p()
+    _check("abm_create", lib().abm_create(params, n_particles, n_param_sets, seed, C.byref(h)))
+    return h
+
+
+def abm_step(ctx, n_steps):
+    _check("abm_step", lib().abm_step(ctx, n_steps))
+
+
+def abm_snapshot(ctx, dev_ptr, stride_bytes):
+    _check("abm_snapshot", lib().abm_snapshot(ctx, dev_ptr, stride_bytes))
+
+
+def abm_snapshot_host(ctx, host_array, stride_bytes):
+    _check("abm_snapshot_host", lib().abm_snapshot_host(ctx, host_array.ctypes.data, stride_bytes))
+
+
+def abm_moments(ctx, n_param_sets):
+    out = np.zeros(n_param_sets, MOMENT_DTYPE)
+    _check("abm_moments", lib().abm_moments(ctx, out.ctypes.data))
+    return out
+
+
+def abm_moment_sums(ctx, n_param_sets):
+    out = np.zeros((n_param_sets, ABM_N_SUMS), np.float64)
+    _check("abm_moment_sums", lib().abm_moment_sums(ctx, out.ctypes.data))
+    return out
+
+
+def abm_moments_from_sums(sums, step):
+    sums = np.ascontiguousarray(sums, np.float64)
+    out = np.zeros(sums.shape[0], MOMENT_DTYPE)
+    _check("abm_moments_from_sums",
+           lib().abm_moments_from_sums(sums.ctypes.data, sums.shape[0], step, out.ctypes.data))
+    return out
+
+
+def abm_get_step(ctx):
+    n = C.c_uint64()
+    _check("abm_get_step", lib().abm_get_step(ctx, C.byref(n)))
+    return n.value
+
+
+def abm_destroy(ctx):
+    _check("abm_destroy", lib().abm_destroy(ctx))
+
+
+def abm_philox_blocks(seed, traj_first, n_traj, block_first, n_blocks, dev_ptr, stream=0):
+    _check("abm_philox_blocks",
+           lib().abm_philox_blocks(seed, traj_first, n_traj, block_first & 0xffffffffffffffff,
+                                   n_blocks, dev_ptr, stream or None))
+
+
+# ---- convenience wrapper (owns the handle and the torch snapshot buffer) ----------------------
+
+class Ensemble:
+    """A context plus the caller-owned device snapshot buffer (a torch tensor).
+
+    `param_sets`: list of parameter dicts (workloads.Workload.set_params), or an abm_params
+    array from make_params (then stream / snapshot_every / traj_base must already be set in it).
+    Marshalling only.
+    """
+
+    def __init__(self, param_sets, n_particles, seed, snapshot_every=0, stream=None,
+                 traj_base=0, traj_set_stride=0):
+        import torch
+        self._torch = torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1104_2499_b200 needs a CUDA device (no CPU fallback)")
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self.n_sets = len(param_sets)
+        self.n_particles = n_particles
+        self.n_traj = n_particles * self.n_sets
+        if isinstance(param_sets, C.Array):      # already marshalled (make_params) by the caller
+            params = param_sets
+        else:
+            params = make_params(param_sets, stream=self.stream.cuda_stream,
+                                 snapshot_every=snapshot_every, traj_base=traj_base,
+                                 traj_set_stride=traj_set_stride)
+        self.fp64 = int(params[0].precision) == 1
+        self.ctx = abm_create(params, n_particles, self.n_sets, seed)
+        self.frame = None
+
+    def bind_snapshot(self, with_e=False):
+        """Allocate (once) and bind a device frame: [n_traj, 2] (x, v) or [n_traj, 4] (x, v, e, 1)."""
+        torch = self._torch
+        cols = 4 if with_e else 2
+        dtype = torch.float64 if self.fp64 else torch.float32
+        if self.frame is None or self.frame.shape[1] != cols:
+            with torch.cuda.stream(self.stream):
+                self.frame = torch.empty((self.n_traj, cols), dtype=dtype, device="cuda")
+        abm_snapshot(self.ctx, self.frame.data_ptr(), cols * self.frame.element_size())
+        return self.frame
+
+    def unbind_snapshot(self):
+        abm_snapshot(self.ctx, None, 0)
+
+    def step(self, n):
+        abm_step(self.ctx, n)
+
+    def moments(self):
+        return abm_moments(self.ctx, self.n_sets)
+
+    def moment_sums(self):
+        return abm_moment_sums(self.ctx, self.n_sets)
+
+    def state(self):
+        """Current (x, v, e) of all trajectories as a float64 numpy array [n_traj, 3] (host)."""
+        cols, item = 4, (8 if self.fp64 else 4)
+        host = np.empty((self.n_traj, cols), np.float64 if self.fp64 else np.float32)
+        abm_snapshot_host(self.ctx, host, cols * item)
+        return host[:, :3].astype(np.float64)
+
+    @property
+    def step_count(self):
+        return abm_get_step(self.ctx)
+
+    def close(self):
+        if self.ctx is not None:
+            abm_destroy(self.ctx)
+            self.ctx = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,465 @@
+// abm.cu -- host side of the C ABI declared in include/abm.h.
+//
+// Owns the context (state arrays, coefficient table, reduction scratch), precomputes the
+// per-set coefficients in fp64, and enqueues the kernels of abm_kernels.cuh on the caller's
+// stream.  There is no CPU fallback: every step of the path runs in those kernels.
+#include "abm.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "abm_kernels.cuh"
+
+namespace {
+
+using namespace abm;
+
+constexpr uint32_t CTX_MAGIC = 0x41424d31u;      // "ABM1"
+constexpr uint32_t MAX_LAUNCH_STEPS = 1u << 30;  // steps per launch without a tilt table
+constexpr uint32_t TILT_CHUNK = 1u << 16;        // steps per launch with a tilt table
+
+static_assert(sizeof(abm_moment) == 80, "abm_moment is 80 bytes (include/abm.h)");
+static_assert(sizeof(MomentRec) == sizeof(abm_moment), "MomentRec mirrors abm_moment");
+static_assert(N_SUMS == ABM_N_SUMS, "sum count");
+
+}  // namespace
+
+struct abm_ctx {
+  uint32_t magic;
+  int device;
+  cudaStream_t stream;
+  uint32_t precision, integrator, init_v, snap_every;
+  uint32_t n_sets;
+  bool tilt;
+  uint64_t n_particles, n_traj, seed, step, traj_base, set_stride;
+  double dt, omega;
+  size_t real_size;
+  void *x, *v, *e;      // state, SoA, Real[n_traj]
+  void* coef_table;     // Coef<Real>[n_sets]
+  void* tilt_table;     // Real[TILT_CHUNK + 1]
+  double* partial;      // [n_sets * blocks_per_set][7]
+  double* sums;         // [n_sets][8]
+  MomentRec* moments;   // [n_sets]
+  void* frame;          // staging frame for abm_snapshot_host (lazily allocated)
+  size_t frame_bytes;
+  uint32_t mom_block, mom_slice, blocks_per_set;
+  void* snap;
+  uint32_t snap_stride;
+  int sticky;           // first CUDA error seen
+  Coef<float> coef0_f;  // set 0 (kernel-parameter copy for single-set runs)
+  Coef<double> coef0_d;
+};
+
+namespace {
+
+#define ABM_CK(ctx, call)                                   \
+  do {                                                      \
+    cudaError_t err__ = (call);                             \
+    if (err__ != cudaSuccess) {                             \
+      if (ctx) (ctx)->sticky = static_cast<int>(err__);     \
+      return err__ == cudaErrorMemoryAllocation ? ABM_ENOMEM : ABM_ECUDA; \
+    }                                                       \
+  } while (0)
+
+template <typename Real>
+Coef<Real> make_coef(const abm_params& p) {
+  const double two_pi = 6.283185307179586476925286766559;
+  Coef<Real> c;
+  std::memset(&c, 0, sizeof(c));
+  c.dt = static_cast<Real>(p.dt);
+  c.hdt = static_cast<Real>(0.5 * p.dt);
+  c.gamma0 = static_cast<Real>(p.gamma0);
+  c.d = static_cast<Real>(p.d);
+  c.q = static_cast<Real>(p.q);
+  c.c = static_cast<Real>(p.c);
+  // -U'(x) = -(2pi/L) (A1 cos th + 2 A2 cos 2th) = (2pi/L) (2 A2 - A1 cos th - 4 A2 cos^2 th)
+  const double g = two_pi / p.L;
+  c.k0 = static_cast<Real>(g * 2.0 * p.A2 + p.F0);
+  c.k1 = static_cast<Real>(-g * p.A1);
+  c.k2 = static_cast<Real>(-g * 4.0 * p.A2);
+  if (sizeof(Real) == 4) {
+    c.th_s = static_cast<Real>(g);                      // radians
+    c.th_o = static_cast<Real>(g * p.phi);
+    c.s2 = static_cast<Real>(-2.0 * (2.0 * p.D * p.dt) * 0.6931471805599453094);  // -2 sigma^2 ln2
+  } else {
+    c.th_s = static_cast<Real>(2.0 / p.L);              // half-turns (cospi)
+    c.th_o = static_cast<Real>(2.0 * p.phi / p.L);
+    c.s2 = static_cast<Real>(std::sqrt(2.0 * p.D * p.dt));  // sigma
+  }
+  c.bm_o = static_cast<Real>(two_pi * 0x1p-24);
+  c.A = static_cast<Real>(p.A);
+  c.L = static_cast<Real>(p.L);
+  c.v0 = static_cast<Real>(p.v0);
+  c.e0 = static_cast<Real>(p.e0);
+  c.sv = static_cast<Real>(p.init_v ? std::sqrt(p.D / p.gamma0) : 0.0);
+  return c;
+}
+
+bool finite_all(const abm_params& p) {
+  const double v[] = {p.dt, p.gamma0, p.q, p.c, p.d, p.D, p.F0, p.A, p.omega,
+                      p.L,  p.A1,     p.A2, p.phi, p.v0, p.e0};
+  for (double t : v)
+    if (!std::isfinite(t)) return false;
+  return true;
+}
+
+int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets) {
+  if (!params || n_particles == 0 || n_sets == 0) return ABM_EINVAL;
+  const abm_params& p0 = params[0];
+  if (p0.struct_size != sizeof(abm_params)) return ABM_EINVAL;
+  if (p0.precision > ABM_FP64 || p0.integrator > ABM_HEUN || p0.init_v > ABM_INIT_V_THERMAL)
+    return ABM_EINVAL;
+  for (uint32_t s = 0; s < n_sets; ++s) {
+    const abm_params& p = params[s];
+    if (p.struct_size != sizeof(abm_params)) return ABM_EINVAL;
+    if (p.precision != p0.precision || p.integrator != p0.integrator || p.init_v != p0.init_v ||
+        p.snapshot_every != p0.snapshot_every || p.dt != p0.dt || p.omega != p0.omega ||
+        p.traj_base != p0.traj_base || p.traj_set_stride != p0.traj_set_stride ||
+        p.stream != p0.stream)
+      return ABM_EINVAL;
+    if (!finite_all(p)) return ABM_EINVAL;
+    if (!(p.dt > 0.0) || !(p.L > 0.0) || p.D < 0.0) return ABM_EINVAL;
+    if (p.init_v == ABM_INIT_V_THERMAL && !(p.gamma0 > 0.0)) return ABM_EINVAL;
+  }
+  // total trajectory count must fit the kernels' 64-bit indexing and 31-bit grids
+  const uint64_t max_traj = static_cast<uint64_t>(0x7fffffffu) * STEP_BLOCK;
+  if (n_particles > max_traj / n_sets) return ABM_EINVAL;
+  if (p0.traj_set_stride != 0 && p0.traj_set_stride < n_particles) return ABM_EINVAL;
+  return ABM_OK;
+}
+
+void free_all(abm_ctx* c) {
+  cudaFree(c->x);
+  cudaFree(c->v);
+  cudaFree(c->e);
+  cudaFree(c->coef_table);
+  cudaFree(c->tilt_table);
+  cudaFree(c->partial);
+  cudaFree(c->sums);
+  cudaFree(c->moments);
+  cudaFree(c->frame);
+}
+
+template <typename Real>
+int upload_coefs_and_init(abm_ctx* c, const abm_params* params) {
+  std::vector<Coef<Real>> tab(c->n_sets);
+  for (uint32_t s = 0; s < c->n_sets; ++s) tab[s] = make_coef<Real>(params[s]);
+  ABM_CK(c, cudaMalloc(&c->coef_table, sizeof(Coef<Real>) * c->n_sets));
+  // synchronous copy from pageable memory: `tab` dies at return
+  ABM_CK(c, cudaMemcpy(c->coef_table, tab.data(), sizeof(Coef<Real>) * c->n_sets,
+                       cudaMemcpyHostToDevice));
+  const uint32_t grid = static_cast<uint32_t>((c->n_traj + 255) / 256);
+  init_kernel<Real><<<grid, 256, 0, c->stream>>>(
+      static_cast<Real*>(c->x), static_cast<Real*>(c->v), static_cast<Real*>(c->e),
+      static_cast<const Coef<Real>*>(c->coef_table), c->n_traj, c->n_particles, c->traj_base,
+      c->set_stride, c->seed, c->n_sets, c->init_v);
+  ABM_CK(c, cudaGetLastError());
+  return ABM_OK;
+}
+
+template <typename Real, int INTEG, bool TILT>
+cudaError_t launch_step_u(const abm_ctx* c, const StepArgs<Real>& a) {
+  const uint32_t grid = static_cast<uint32_t>((c->n_traj + STEP_BLOCK - 1) / STEP_BLOCK);
+  if (c->n_sets == 1)
+    step_kernel<Real, INTEG, TILT, true><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+  else
+    step_kernel<Real, INTEG, TILT, false><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+  return cudaGetLastError();
+}
+
+template <typename Real>
+cudaError_t launch_step(const abm_ctx* c, const StepArgs<Real>& a) {
+  if (c->integrator == ABM_EULER_MARUYAMA)
+    return c->tilt ? launch_step_u<Real, 0, true>(c, a) : launch_step_u<Real, 0, false>(c, a);
+  return c->tilt ? launch_step_u<Real, 1, true>(c, a) : launch_step_u<Real, 1, false>(c, a);
+}
+
+template <typename Real>
+const Coef<Real>& coef0(const abm_ctx* c);
+template <>
+const Coef<float>& coef0<float>(const abm_ctx* c) { return c->coef0_f; }
+template <>
+const Coef<double>& coef0<double>(const abm_ctx* c) { return c->coef0_d; }
+
+template <typename Real>
+int step_impl(abm_ctx* c, uint64_t n_steps) {
+  StepArgs<Real> a;
+  a.x = static_cast<Real*>(c->x);
+  a.v = static_cast<Real*>(c->v);
+  a.e = static_cast<Real*>(c->e);
+  a.coef_table = static_cast<const Coef<Real>*>(c->coef_table);
+  a.tilt = static_cast<const Real*>(c->tilt_table);
+  a.snap = c->snap;
+  a.n_traj = c->n_traj;
+  a.n_particles = c->n_particles;
+  a.traj_base = c->traj_base;
+  a.set_stride = c->set_stride;
+  a.seed = c->seed;
+  a.snap_every = c->snap_every;
+  a.snap_stride = c->snap_stride;
+  a.coef0 = coef0<Real>(c);
+  const uint32_t chunk_max = c->tilt ? TILT_CHUNK : MAX_LAUNCH_STEPS;
+  while (n_steps > 0) {
+    const uint32_t chunk = static_cast<uint32_t>(n_steps < chunk_max ? n_steps : chunk_max);
+    a.step0 = c->step;
+    a.tilt_base = c->step;
+    a.n_steps = chunk;
+    if (c->tilt) {
+      const uint32_t n_tab = chunk + 1;  // Heun reads t_{n+1} of the last step
+      tilt_kernel<Real><<<(n_tab + 255) / 256, 256, 0, c->stream>>>(
+          static_cast<Real*>(c->tilt_table), c->step, n_tab, c->omega, c->dt);
+      ABM_CK(c, cudaGetLastError());
+    }
+    ABM_CK(c, launch_step<Real>(c, a));
+    c->step += chunk;
+    n_steps -= chunk;
+  }
+  return ABM_OK;
+}
+
+template <typename Real>
+int reduce_moments(abm_ctx* c) {
+  const uint32_t grid = c->n_sets * c->blocks_per_set;
+  moments_partial_kernel<Real><<<grid, c->mom_block, 0, c->stream>>>(
+      static_cast<const Real*>(c->x), static_cast<const Real*>(c->v),
+      static_cast<const Real*>(c->e), static_cast<const Coef<Real>*>(c->coef_table),
+      c->n_particles, c->traj_base, c->set_stride, c->seed, c->blocks_per_set, c->mom_slice,
+      c->partial);
+  ABM_CK(c, cudaGetLastError());
+  moments_final_kernel<<<(c->n_sets + 127) / 128, 128, 0, c->stream>>>(
+      c->partial, c->n_sets, c->blocks_per_set, c->n_particles, c->step, c->sums, c->moments);
+  ABM_CK(c, cudaGetLastError());
+  return ABM_OK;
+}
+
+int check_ctx(const abm_ctx* c) {
+  if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
+  if (c->sticky) return ABM_ECUDA;
+  return ABM_OK;
+}
+
+bool stride_ok(const abm_ctx* c, size_t stride) {
+  return c->precision == ABM_FP32 ? (stride == 8 || stride == 16) : (stride == 16 || stride == 32);
+}
+
+int write_frame(abm_ctx* c, void* dev_ptr, uint32_t stride) {
+  const uint32_t grid = static_cast<uint32_t>((c->n_traj + 255) / 256);
+  if (c->precision == ABM_FP32)
+    snapshot_kernel<float><<<grid, 256, 0, c->stream>>>(
+        static_cast<const float*>(c->x), static_cast<const float*>(c->v),
+        static_cast<const float*>(c->e), c->n_traj, dev_ptr, stride);
+  else
+    snapshot_kernel<double><<<grid, 256, 0, c->stream>>>(
+        static_cast<const double*>(c->x), static_cast<const double*>(c->v),
+        static_cast<const double*>(c->e), c->n_traj, dev_ptr, stride);
+  ABM_CK(c, cudaGetLastError());
+  return ABM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_sets,
+               uint64_t seed, abm_ctx** out) {
+  if (!out) return ABM_EINVAL;
+  const int vs = validate(params, n_particles, n_param_sets);
+  if (vs != ABM_OK) return vs;
+  int device = -1;
+  if (cudaGetDevice(&device) != cudaSuccess) return ABM_ECUDA;  // no device: fail loudly
+  abm_ctx* c = new (std::nothrow) abm_ctx;
+  if (!c) return ABM_ENOMEM;
+  std::memset(static_cast<void*>(c), 0, sizeof(*c));
+  const abm_params& p0 = params[0];
+  c->magic = CTX_MAGIC;
+  c->device = device;
+  c->stream = static_cast<cudaStream_t>(p0.stream);
+  c->precision = p0.precision;
+  c->integrator = p0.integrator;
+  c->init_v = p0.init_v;
+  c->snap_every = p0.snapshot_every;
+  c->n_sets = n_param_sets;
+  c->n_particles = n_particles;
+  c->n_traj = n_particles * n_param_sets;
+  c->seed = seed;
+  c->step = 0;
+  c->traj_base = p0.traj_base;
+  c->set_stride = p0.traj_set_stride ? p0.traj_set_stride : n_particles;
+  c->dt = p0.dt;
+  c->omega = p0.omega;
+  c->tilt = false;
+  for (uint32_t s = 0; s < n_param_sets; ++s)
+    if (params[s].A != 0.0) c->tilt = true;
+  c->real_size = c->precision == ABM_FP32 ? 4 : 8;
+  c->coef0_f = make_coef<float>(p0);
+  c->coef0_d = make_coef<double>(p0);
+
+  // moment reduction geometry: one CTA per slice of a set
+  uint32_t mb = MOM_BLOCK;
+  if (n_particles < MOM_BLOCK) mb = static_cast<uint32_t>((n_particles + 31) / 32 * 32);
+  c->mom_block = mb;
+  c->mom_slice = mb * MOM_PER_THREAD;
+  const uint64_t bps = (n_particles + c->mom_slice - 1) / c->mom_slice;
+  if (bps * n_param_sets > 0x7fffffffull) {
+    delete c;
+    return ABM_EINVAL;
+  }
+  c->blocks_per_set = static_cast<uint32_t>(bps);
+
+  int rc = ABM_OK;
+  auto fail = [&](int code) {
+    free_all(c);
+    c->magic = 0;
+    delete c;
+    return code;
+  };
+  auto alloc = [&](void** p, size_t bytes) {
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+      rc = e == cudaErrorMemoryAllocation ? ABM_ENOMEM : ABM_ECUDA;
+      cudaGetLastError();
+      return false;
+    }
+    return true;
+  };
+  const size_t state_bytes = c->real_size * c->n_traj;
+  if (!alloc(&c->x, state_bytes) || !alloc(&c->v, state_bytes) || !alloc(&c->e, state_bytes) ||
+      !alloc(reinterpret_cast<void**>(&c->partial),
+             sizeof(double) * (N_SUMS - 1) * bps * n_param_sets) ||
+      !alloc(reinterpret_cast<void**>(&c->sums), sizeof(double) * N_SUMS * n_param_sets) ||
+      !alloc(reinterpret_cast<void**>(&c->moments), sizeof(MomentRec) * n_param_sets) ||
+      (c->tilt && !alloc(&c->tilt_table, c->real_size * (TILT_CHUNK + 1))))
+    return fail(rc);
+  rc = c->precision == ABM_FP32 ? upload_coefs_and_init<float>(c, params)
+                                : upload_coefs_and_init<double>(c, params);
+  if (rc != ABM_OK) return fail(rc);
+  *out = c;
+  return ABM_OK;
+}
+
+int abm_step(abm_ctx* c, uint64_t n_steps) {
+  const int st = check_ctx(c);
+  if (st != ABM_OK) return st;
+  if (n_steps == 0) return ABM_OK;
+  return c->precision == ABM_FP32 ? step_impl<float>(c, n_steps) : step_impl<double>(c, n_steps);
+}
+
+int abm_snapshot(abm_ctx* c, void* dev_ptr, size_t stride_bytes) {
+  const int st = check_ctx(c);
+  if (st != ABM_OK) return st;
+  if (!dev_ptr) {
+    c->snap = nullptr;
+    c->snap_stride = 0;
+    return ABM_OK;
+  }
+  if (!stride_ok(c, stride_bytes)) return ABM_EINVAL;
+  if (reinterpret_cast<uintptr_t>(dev_ptr) % stride_bytes != 0) return ABM_EINVAL;
+  const int rc = write_frame(c, dev_ptr, static_cast<uint32_t>(stride_bytes));
+  if (rc != ABM_OK) return rc;
+  c->snap = dev_ptr;
+  c->snap_stride = static_cast<uint32_t>(stride_bytes);
+  return ABM_OK;
+}
+
+int abm_snapshot_host(abm_ctx* c, void* host_ptr, size_t stride_bytes) {
+  const int st = check_ctx(c);
+  if (st != ABM_OK) return st;
+  if (!host_ptr || !stride_ok(c, stride_bytes)) return ABM_EINVAL;
+  const size_t bytes = stride_bytes * c->n_traj;
+  if (c->frame_bytes < bytes) {
+    ABM_CK(c, cudaStreamSynchronize(c->stream));
+    cudaFree(c->frame);
+    c->frame = nullptr;
+    c->frame_bytes = 0;
+    ABM_CK(c, cudaMalloc(&c->frame, bytes));
+    c->frame_bytes = bytes;
+  }
+  const int rc = write_frame(c, c->frame, static_cast<uint32_t>(stride_bytes));
+  if (rc != ABM_OK) return rc;
+  ABM_CK(c, cudaMemcpyAsync(host_ptr, c->frame, bytes, cudaMemcpyDeviceToHost, c->stream));
+  ABM_CK(c, cudaStreamSynchronize(c->stream));
+  return ABM_OK;
+}
+
+int abm_moments(abm_ctx* c, abm_moment* out) {
+  const int st = check_ctx(c);
+  if (st != ABM_OK) return st;
+  if (!out) return ABM_EINVAL;
+  const int rc = c->precision == ABM_FP32 ? reduce_moments<float>(c) : reduce_moments<double>(c);
+  if (rc != ABM_OK) return rc;
+  ABM_CK(c, cudaMemcpyAsync(out, c->moments, sizeof(abm_moment) * c->n_sets,
+                            cudaMemcpyDeviceToHost, c->stream));
+  ABM_CK(c, cudaStreamSynchronize(c->stream));
+  return ABM_OK;
+}
+
+int abm_moment_sums(abm_ctx* c, double* out) {
+  const int st = check_ctx(c);
+  if (st != ABM_OK) return st;
+  if (!out) return ABM_EINVAL;
+  const int rc = c->precision == ABM_FP32 ? reduce_moments<float>(c) : reduce_moments<double>(c);
+  if (rc != ABM_OK) return rc;
+  ABM_CK(c, cudaMemcpyAsync(out, c->sums, sizeof(double) * N_SUMS * c->n_sets,
+                            cudaMemcpyDeviceToHost, c->stream));
+  ABM_CK(c, cudaStreamSynchronize(c->stream));
+  return ABM_OK;
+}
+
+int abm_moments_from_sums(const double* sums, uint32_t n_param_sets, uint64_t step,
+                          abm_moment* out_moments) {
+  if (!sums || !out_moments || n_param_sets == 0) return ABM_EINVAL;
+  for (uint32_t s = 0; s < n_param_sets; ++s) {
+    if (!(sums[static_cast<size_t>(s) * N_SUMS] >= 1.0)) return ABM_EINVAL;
+    MomentRec m;
+    finalize_moment(sums + static_cast<size_t>(s) * N_SUMS, step, &m);
+    std::memcpy(&out_moments[s], &m, sizeof(m));
+  }
+  return ABM_OK;
+}
+
+int abm_get_step(const abm_ctx* c, uint64_t* out_step) {
+  if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
+  if (!out_step) return ABM_EINVAL;
+  *out_step = c->step;
+  return ABM_OK;
+}
+
+int abm_destroy(abm_ctx* c) {
+  if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
+  cudaStreamSynchronize(c->stream);
+  free_all(c);
+  c->magic = 0;
+  delete c;
+  return ABM_OK;
+}
+
+int abm_philox_blocks(uint64_t seed, uint64_t traj_first, uint64_t n_traj, uint64_t block_first,
+                      uint64_t n_blocks, uint32_t* dev_out, void* stream) {
+  if (!dev_out || n_traj == 0 || n_blocks == 0) return ABM_EINVAL;
+  if (reinterpret_cast<uintptr_t>(dev_out) % 16 != 0) return ABM_EINVAL;
+  if (n_traj > (0x7fffffffull * 256) / n_blocks) return ABM_EINVAL;
+  const uint64_t total = n_traj * n_blocks;
+  philox_blocks_kernel<<<static_cast<uint32_t>((total + 255) / 256), 256, 0,
+                         static_cast<cudaStream_t>(stream)>>>(
+      seed, traj_first, n_traj, block_first, n_blocks, reinterpret_cast<uint4*>(dev_out));
+  return cudaGetLastError() == cudaSuccess ? ABM_OK : ABM_ECUDA;
+}
+
+const char* abm_strerror(int status) {
+  switch (status) {
+    case ABM_OK: return "ok";
+    case ABM_EINVAL: return "invalid argument";
+    case ABM_ENOMEM: return "out of memory";
+    case ABM_ECUDA: return "CUDA error (no usable device, or a launch/copy failed)";
+    case ABM_ESTATE: return "null or destroyed context";
+    default: return "unknown status";
+  }
+}
+
+uint32_t abm_abi_version(void) { return 1; }
+
+}  // extern "C"

@@ -1,0 +1,230 @@
+// abm_device.cuh -- device-side building blocks of the hot path (sm_100a).
+//
+// S1 Philox4x32-10 block, S2 Box-Muller, S3 force, S4 Euler-Maruyama / stochastic Heun update
+// (Fig. 1 loop body, Eqs. 1-3 at PAPER.md:59-69).
+//
+// Everything is written with explicit fma/mul/add intrinsics so that the unrolled 4-step path
+// and the single-step path of the step kernel round identically (abm_step(a); abm_step(b) must
+// be bit-identical to abm_step(a+b)).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace abm {
+
+// ---------------------------------------------------------------------------------------------
+// S1  Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), restated from the published round
+// function: (hi0,lo0) = M0*c0, (hi1,lo1) = M1*c2, c' = (hi1^c1^k0, lo1, hi0^c3^k1, lo0),
+// key += (W0, W1) after each round.
+// ---------------------------------------------------------------------------------------------
+constexpr uint32_t PHILOX_M0 = 0xD2511F53u;
+constexpr uint32_t PHILOX_M1 = 0xCD9E8D57u;
+constexpr uint32_t PHILOX_W0 = 0x9E3779B9u;
+constexpr uint32_t PHILOX_W1 = 0xBB67AE85u;
+
+// 32 x 32 -> 64 multiply as ONE IMAD.WIDE.U32 (the C++ form `uint64_t(a) * M` makes ptxas add
+// a zero high-word correction after every product).
+__device__ __forceinline__ void mul_wide(uint32_t a, uint32_t m, uint32_t& hi, uint32_t& lo) {
+  asm("{\n\t.reg .u64 p;\n\tmul.wide.u32 p, %2, %3;\n\tmov.b64 {%0, %1}, p;\n\t}"
+      : "=r"(lo), "=r"(hi)
+      : "r"(a), "r"(m));
+}
+
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0, lo0, hi1, lo1;
+    mul_wide(c0, PHILOX_M0, hi0, lo0);
+    mul_wide(c2, PHILOX_M1, hi1, lo1);
+    c0 = hi1 ^ c1 ^ (k0 + PHILOX_W0 * static_cast<uint32_t>(r));  // LOP3 with a uniform operand
+    c1 = lo1;
+    c2 = hi0 ^ c3 ^ (k1 + PHILOX_W1 * static_cast<uint32_t>(r));
+    c3 = lo0;
+  }
+  return make_uint4(c0, c1, c2, c3);
+}
+
+// Stream layout: key = (seed lo, seed hi),
+// ctr = (block lo, block hi, trajectory lo, trajectory hi).
+__device__ __forceinline__ uint4 philox_block(uint64_t seed, uint64_t traj, uint64_t b) {
+  return philox4x32_10(static_cast<uint32_t>(b), static_cast<uint32_t>(b >> 32),
+                       static_cast<uint32_t>(traj), static_cast<uint32_t>(traj >> 32),
+                       static_cast<uint32_t>(seed), static_cast<uint32_t>(seed >> 32));
+}
+
+constexpr uint64_t INIT_BLOCK = 0xFFFFFFFFFFFFFFFFull;  // block index of the init block
+
+// ---------------------------------------------------------------------------------------------
+// Approximate single-precision special functions: one MUFU each (plus the range-scale FMUL the
+// hardware wants in front of SIN/COS).  .ftz keeps ptxas from adding denormal fix-up code.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float fast_lg2(float x) {
+  float y;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float fast_sqrt(float x) {
+  float y;
+  asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float fast_cos(float x) {
+  float y;
+  asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float fast_sin(float x) {
+  float y;
+  asm("sin.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Per-parameter-set coefficients, precomputed in fp64 on the host and rounded once.
+// ---------------------------------------------------------------------------------------------
+template <typename Real>
+struct Coef {
+  Real dt, hdt;        // dt, dt/2
+  Real gamma0, d, q, c;
+  Real k0, k1, k2;     // -U'(x) + F0 = k0 + k1 cos(th) + k2 cos(th)^2
+  Real th_s, th_o;     // fp32: th = th_s x + th_o [rad];  fp64: th/pi = th_s x + th_o
+  Real s2;             // fp32: -2 sigma^2 ln 2 (so sigma^2 (-2 ln u) = s2 lg2 u); fp64: sigma
+  Real A;              // tilt amplitude
+  Real L, v0, e0, sv;  // init: x0 = L u, v0, e0, sv = sqrt(D/gamma0)
+  Real bm_o;           // fp32: 2 pi 2^-24, the half-ulp offset of the Box-Muller angle
+  Real pad[2];
+};
+static_assert(sizeof(Coef<float>) == 80, "Coef<float> layout");
+static_assert(sizeof(Coef<double>) == 160, "Coef<double> layout");
+
+template <typename Real>
+struct State {
+  Real x, v, e;
+};
+
+// ---------------------------------------------------------------------------------------------
+// S2  Box-Muller on a word pair -> (rho, cos, sin) with rho = sigma sqrt(-2 ln u1) so that
+// sigma z_even = rho cos(2 pi u2), sigma z_odd = rho sin(2 pi u2).
+// fp32 uniform map ((w >> 9) + 0.5) 2^-23, built exactly as m - (1 - 2^-24) with
+// m = as_float((w >> 9) + 0x3f800000) in [1, 2).
+// ---------------------------------------------------------------------------------------------
+struct Normal2f {
+  float rho, cs, sn;
+};
+
+__device__ __forceinline__ float uniform_f32(uint32_t w) {
+  const float m = __uint_as_float((w >> 9) + 0x3f800000u);
+  return __fadd_rn(m, -(1.0f - 0x1p-24f));  // exact
+}
+
+__device__ __forceinline__ Normal2f box_muller_f32(uint32_t wa, uint32_t wb, float s2,
+                                                   float bm_o) {
+  Normal2f o;
+  const float u1 = uniform_f32(wa);
+  o.rho = fast_sqrt(__fmul_rn(fast_lg2(u1), s2));
+  // angle 2 pi u2 = 2 pi (m - 1 + 2^-24), m in [1, 2): the "- 2 pi" is a whole turn, so one FMA
+  const float m2 = __uint_as_float((wb >> 9) + 0x3f800000u);
+  const float ang = __fmaf_rn(m2, 6.283185307179586f, bm_o);
+  o.cs = fast_cos(ang);
+  o.sn = fast_sin(ang);
+  return o;
+}
+
+struct Normal2d {
+  double rho, cs, sn;
+};
+
+__device__ __forceinline__ double uniform_f64(uint32_t w) {
+  return __fma_rn(static_cast<double>(w), 0x1p-32, 0x1p-33);  // (w + 0.5) 2^-32, exact
+}
+
+__device__ __forceinline__ Normal2d box_muller_f64(uint32_t wa, uint32_t wb, double sigma) {
+  Normal2d o;
+  o.rho = __dmul_rn(sigma, sqrt(__dmul_rn(-2.0, log(uniform_f64(wa)))));
+  sincospi(__dmul_rn(2.0, uniform_f64(wb)), &o.sn, &o.cs);
+  return o;
+}
+
+// ---------------------------------------------------------------------------------------------
+// S3  force  -U'(x) + F0 (+ tilt folded into k0t by the caller):  one cosine per evaluation,
+// cos 2th = 2 cos^2 th - 1  (Eq. 3).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float force(const Coef<float>& k, float x, float k0t) {
+  const float c = fast_cos(__fmaf_rn(x, k.th_s, k.th_o));
+  return __fmaf_rn(__fmaf_rn(k.k2, c, k.k1), c, k0t);
+}
+__device__ __forceinline__ double force(const Coef<double>& k, double x, double k0t) {
+  const double c = cospi(__fma_rn(x, k.th_s, k.th_o));
+  return __fma_rn(__fma_rn(k.k2, c, k.k1), c, k0t);
+}
+
+__device__ __forceinline__ float fma_(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return __fma_rn(a, b, c); }
+__device__ __forceinline__ float mul_(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float add_(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_(double a, double b) { return __dadd_rn(a, b); }
+
+// ---------------------------------------------------------------------------------------------
+// S4  one step.  k0t = k0 + A cos(omega t_n), k0t1 = k0 + A cos(omega t_{n+1}) (Heun only);
+// (rho, cs) = noise of this step, sigma z = rho * cs.
+//
+// Euler-Maruyama (all right-hand sides at the old state, reading G4):
+//   x' = x + dt v;  v' = v + dt a_v + sigma z;  e' = e + dt a_e
+//   a_v = (d e - gamma0) v + f(x),   a_e = q - e (c + d v^2)             (Eqs. 2, 1)
+// The increments are added to the state unscaled (no pre-multiplied (1 - gamma0 dt) factors):
+// a rounded factor next to 1 would bias every step in the same direction.
+// ---------------------------------------------------------------------------------------------
+template <typename Real>
+__device__ __forceinline__ void em_step(State<Real>& s, const Coef<Real>& k, Real k0t, Real rho,
+                                        Real cs) {
+  const Real f = force(k, s.x, k0t);
+  const Real av = fma_(fma_(k.d, s.e, -k.gamma0), s.v, f);
+  const Real ae = fma_(-s.e, fma_(k.d, mul_(s.v, s.v), k.c), k.q);
+  s.x = fma_(k.dt, s.v, s.x);
+  s.v = fma_(rho, cs, fma_(k.dt, av, s.v));
+  s.e = fma_(k.dt, ae, s.e);
+}
+
+// Stochastic Heun: predictor = EM step with the full noise increment; corrector averages the
+// drift at (X, t_n) and (X~, t_{n+1}); the same sigma z in both (reading G16).
+template <typename Real>
+__device__ __forceinline__ void heun_step(State<Real>& s, const Coef<Real>& k, Real k0t, Real k0t1,
+                                          Real rho, Real cs) {
+  const Real sz = mul_(rho, cs);
+  const Real f1 = force(k, s.x, k0t);
+  const Real av1 = fma_(fma_(k.d, s.e, -k.gamma0), s.v, f1);
+  const Real ae1 = fma_(-s.e, fma_(k.d, mul_(s.v, s.v), k.c), k.q);
+  const Real xp = fma_(k.dt, s.v, s.x);
+  const Real vp = add_(fma_(k.dt, av1, s.v), sz);
+  const Real ep = fma_(k.dt, ae1, s.e);
+  const Real f2 = force(k, xp, k0t1);
+  const Real av2 = fma_(fma_(k.d, ep, -k.gamma0), vp, f2);
+  const Real ae2 = fma_(-ep, fma_(k.d, mul_(vp, vp), k.c), k.q);
+  s.x = fma_(k.hdt, add_(s.v, vp), s.x);
+  s.v = add_(fma_(k.hdt, add_(av1, av2), s.v), sz);
+  s.e = fma_(k.hdt, add_(ae1, ae2), s.e);
+}
+
+// ---------------------------------------------------------------------------------------------
+// S0  initial state from the init block: x0 = L u(w0) with the run's position map,
+// v0 constant or sv * sqrt(-2 ln u(w2)) cos(2 pi u(w3)), e0 constant; w1 reserved.
+// Not on the hot loop: precise functions.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float init_x(const Coef<float>& k, uint32_t w0) {
+  return __fmul_rn(k.L, __fmul_rn(static_cast<float>(w0 >> 8), 0x1p-24f));
+}
+__device__ __forceinline__ double init_x(const Coef<double>& k, uint32_t w0) {
+  return __dmul_rn(k.L, __dmul_rn(static_cast<double>(w0), 0x1p-32));
+}
+__device__ __forceinline__ float init_v_thermal(const Coef<float>& k, uint32_t w2, uint32_t w3) {
+  const float r = sqrtf(-2.0f * logf(uniform_f32(w2)));
+  return k.sv * r * cospif(2.0f * uniform_f32(w3));
+}
+__device__ __forceinline__ double init_v_thermal(const Coef<double>& k, uint32_t w2, uint32_t w3) {
+  const double r = sqrt(-2.0 * log(uniform_f64(w2)));
+  return k.sv * r * cospi(2.0 * uniform_f64(w3));
+}
+
+}  // namespace abm

@@ -1,0 +1,332 @@
+// abm_kernels.cuh -- the kernels of the hot path (sm_100a): init (S0), step (S1-S5, S7),
+// snapshot (S5), moments (S6), tilt table and the Philox diagnostic.
+#pragma once
+#include "abm_device.cuh"
+
+namespace abm {
+
+constexpr int STEP_BLOCK = 128;   // threads per CTA of the step kernel
+constexpr int STEP_MIN_BLOCKS = 12;  // resident CTAs per SM the register budget allows (40 regs)
+constexpr int MOM_BLOCK = 256;    // threads per CTA of the moment reduction (max)
+constexpr int MOM_PER_THREAD = 16;
+constexpr int N_SUMS = 8;
+
+template <typename Real>
+struct StepArgs {
+  Real* x;
+  Real* v;
+  Real* e;
+  const Coef<Real>* coef_table;  // [n_sets] (used when !UNIFORM)
+  const Real* tilt;              // tilt[j] = cos(omega (tilt_base + j) dt) (used when TILT)
+  void* snap;                    // bound snapshot buffer or nullptr
+  uint64_t n_traj;               // local trajectories
+  uint64_t n_particles;          // per set
+  uint64_t traj_base, set_stride;
+  uint64_t seed;
+  uint64_t step0;                // first global step of this launch
+  uint64_t tilt_base;            // global step of tilt[0]
+  uint32_t n_steps;              // steps in this launch
+  uint32_t snap_every;           // K (0 = never)
+  uint32_t snap_stride;          // bytes per trajectory in snap
+  Coef<Real> coef0;              // the single set's coefficients (used when UNIFORM)
+};
+
+// ---------------------------------------------------------------------------------------------
+// index helpers
+// ---------------------------------------------------------------------------------------------
+struct TrajId {
+  uint64_t global;  // index into the random stream
+  uint32_t set;
+};
+__device__ __forceinline__ TrajId traj_id(uint64_t k, uint64_t n_particles, uint64_t traj_base,
+                                          uint64_t set_stride, bool single_set) {
+  TrajId t;
+  if (single_set) {
+    t.set = 0;
+    t.global = traj_base + k;
+  } else {
+    const uint64_t s = k / n_particles;
+    t.set = static_cast<uint32_t>(s);
+    t.global = traj_base + s * set_stride + (k - s * n_particles);
+  }
+  return t;
+}
+
+// ---------------------------------------------------------------------------------------------
+// S5  snapshot store: float2 (x, v) / float4 (x, v, e, 1) per trajectory, thread-contiguous so
+// a warp writes 256 / 512 contiguous bytes (the headless stand-in for the GL vertex buffer,
+// PAPER.md:158-162).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void store_snapshot(void* snap, uint32_t stride, uint64_t k,
+                                               const State<float>& s) {
+  if (stride == 8) {
+    reinterpret_cast<float2*>(snap)[k] = make_float2(s.x, s.v);
+  } else {
+    reinterpret_cast<float4*>(snap)[k] = make_float4(s.x, s.v, s.e, 1.0f);
+  }
+}
+__device__ __forceinline__ void store_snapshot(void* snap, uint32_t stride, uint64_t k,
+                                               const State<double>& s) {
+  if (stride == 16) {
+    reinterpret_cast<double2*>(snap)[k] = make_double2(s.x, s.v);
+  } else {
+    reinterpret_cast<double4*>(snap)[k] = make_double4(s.x, s.v, s.e, 1.0);
+  }
+}
+
+template <typename Real>
+__global__ void snapshot_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
+                                const Real* __restrict__ e, uint64_t n_traj, void* snap,
+                                uint32_t stride) {
+  const uint64_t k = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (k >= n_traj) return;
+  State<Real> s{x[k], v[k], e[k]};
+  store_snapshot(snap, stride, k, s);
+}
+
+// ---------------------------------------------------------------------------------------------
+// S0  init
+// ---------------------------------------------------------------------------------------------
+template <typename Real>
+__global__ void init_kernel(Real* __restrict__ x, Real* __restrict__ v, Real* __restrict__ e,
+                            const Coef<Real>* __restrict__ coef_table, uint64_t n_traj,
+                            uint64_t n_particles, uint64_t traj_base, uint64_t set_stride,
+                            uint64_t seed, uint32_t n_sets, uint32_t init_v) {
+  const uint64_t k = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (k >= n_traj) return;
+  const TrajId id = traj_id(k, n_particles, traj_base, set_stride, n_sets == 1);
+  const Coef<Real> c = coef_table[id.set];
+  const uint4 w = philox_block(seed, id.global, INIT_BLOCK);
+  x[k] = init_x(c, w.x);
+  v[k] = init_v ? init_v_thermal(c, w.z, w.w) : c.v0;
+  e[k] = c.e0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// tilt table: tilt[j] = cos(omega * ((base + j) * dt)), evaluated in fp64 (reading G15)
+// ---------------------------------------------------------------------------------------------
+template <typename Real>
+__global__ void tilt_kernel(Real* __restrict__ tilt, uint64_t base, uint32_t n, double omega,
+                            double dt) {
+  const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= n) return;
+  const double t = static_cast<double>(base + j) * dt;
+  tilt[j] = static_cast<Real>(cos(omega * t));
+}
+
+// ---------------------------------------------------------------------------------------------
+// The step kernel.  One trajectory per thread; the state lives in registers for the whole
+// launch ("fill local memory with parameters ... for i = 0 to T ... assign local
+// parameters to global memory").  One Philox block feeds four steps: words (0,1) -> steps
+// 4b, 4b+1 (cos, sin), words (2,3) -> steps 4b+2, 4b+3.
+// ---------------------------------------------------------------------------------------------
+template <typename Real>
+struct Noise4;
+template <>
+struct Noise4<float> {
+  Normal2f a, b;
+  __device__ __forceinline__ Noise4(const uint4& w, const Coef<float>& k)
+      : a(box_muller_f32(w.x, w.y, k.s2, k.bm_o)), b(box_muller_f32(w.z, w.w, k.s2, k.bm_o)) {}
+};
+template <>
+struct Noise4<double> {
+  Normal2d a, b;
+  __device__ __forceinline__ Noise4(const uint4& w, const Coef<double>& k)
+      : a(box_muller_f64(w.x, w.y, k.s2)), b(box_muller_f64(w.z, w.w, k.s2)) {}
+};
+
+template <typename Real, int INTEG, bool TILT>
+__device__ __forceinline__ void one_step(State<Real>& s, const Coef<Real>& k, Real rho, Real cs,
+                                         Real t0, Real t1) {
+  const Real k0t = TILT ? fma_(k.A, t0, k.k0) : k.k0;
+  if (INTEG == 0) {
+    em_step(s, k, k0t, rho, cs);
+  } else {
+    const Real k0t1 = TILT ? fma_(k.A, t1, k.k0) : k.k0;
+    heun_step(s, k, k0t, k0t1, rho, cs);
+  }
+}
+
+template <typename Real, int INTEG, bool TILT, bool UNIFORM>
+__global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const __grid_constant__ StepArgs<Real> a) {
+  const uint64_t k = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
+  if (k >= a.n_traj) return;
+  const TrajId id = traj_id(k, a.n_particles, a.traj_base, a.set_stride, UNIFORM);
+  Coef<Real> cf = UNIFORM ? a.coef0 : a.coef_table[id.set];
+  if (UNIFORM) {
+    // Kernel-parameter coefficients are uniform operands and an FMA takes at most one of those.
+    // One operand of each uniform pair -- (d, c), (d, gamma0), (k2, k1), (th_s, th_o) -- and the
+    // Box-Muller angle offset are therefore read from the table in global memory instead: a
+    // loaded value stays in a register for the whole loop, whereas ptxas re-materialises
+    // constant-bank values with an LDC / MOV per use.
+    const Coef<Real>* g = a.coef_table;
+    cf.d = g->d;
+    cf.k1 = g->k1;
+    cf.th_o = g->th_o;
+    cf.bm_o = g->bm_o;
+  }
+
+  State<Real> s{a.x[k], a.v[k], a.e[k]};
+
+  uint64_t n = a.step0;
+  const uint64_t n_end = a.step0 + a.n_steps;
+  const uint32_t K = a.snap != nullptr ? a.snap_every : 0u;
+  uint64_t next_snap = ~0ull;
+  if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
+
+  while (n < n_end) {
+    const uint64_t lim = next_snap < n_end ? next_snap : n_end;
+    if ((n & 3u) == 0 && lim - n >= 4) {
+      // ---- fast path: whole Philox blocks, four steps each ----
+      uint64_t b = n >> 2;
+      uint64_t nb64 = (lim - n) >> 2;
+      const uint64_t to_wrap = 0x100000000ull - (b & 0xffffffffull);  // keep b's high word fixed
+      if (nb64 > to_wrap) nb64 = to_wrap;
+      const uint32_t nb = static_cast<uint32_t>(nb64 > 0x40000000ull ? 0x40000000ull : nb64);
+      const uint32_t b_hi = static_cast<uint32_t>(b >> 32);
+      uint32_t b_lo = static_cast<uint32_t>(b);
+      const Real* tl = TILT ? a.tilt + (n - a.tilt_base) : nullptr;
+      const uint32_t b_end = b_lo + nb;  // may wrap to 0: the loop runs until equality
+#pragma unroll 1
+      do {
+        const uint4 w = philox4x32_10(b_lo, b_hi, static_cast<uint32_t>(id.global),
+                                      static_cast<uint32_t>(id.global >> 32),
+                                      static_cast<uint32_t>(a.seed),
+                                      static_cast<uint32_t>(a.seed >> 32));
+        const Noise4<Real> z(w, cf);
+        Real t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0;
+        if (TILT) {
+          t0 = tl[0]; t1 = tl[1]; t2 = tl[2]; t3 = tl[3];
+          if (INTEG == 1) t4 = tl[4];
+          tl += 4;
+        }
+        one_step<Real, INTEG, TILT>(s, cf, z.a.rho, z.a.cs, t0, t1);
+        one_step<Real, INTEG, TILT>(s, cf, z.a.rho, z.a.sn, t1, t2);
+        one_step<Real, INTEG, TILT>(s, cf, z.b.rho, z.b.cs, t2, t3);
+        one_step<Real, INTEG, TILT>(s, cf, z.b.rho, z.b.sn, t3, t4);
+      } while (++b_lo != b_end);
+      n += static_cast<uint64_t>(nb) << 2;
+    } else {
+      // ---- slow path: one step (unaligned head / tail, or K not a multiple of 4) ----
+      const uint4 w = philox_block(a.seed, id.global, n >> 2);
+      const Noise4<Real> z(w, cf);
+      const bool second = (n >> 1) & 1u;
+      const Real rho = second ? z.b.rho : z.a.rho;
+      const Real cs = (n & 1u) ? (second ? z.b.sn : z.a.sn) : (second ? z.b.cs : z.a.cs);
+      Real t0 = 0, t1 = 0;
+      if (TILT) {
+        t0 = a.tilt[n - a.tilt_base];
+        if (INTEG == 1) t1 = a.tilt[n - a.tilt_base + 1];
+      }
+      one_step<Real, INTEG, TILT>(s, cf, rho, cs, t0, t1);
+      ++n;
+    }
+    if (n == next_snap) {
+      store_snapshot(a.snap, a.snap_stride, k, s);
+      next_snap += K;
+    }
+  }
+  a.x[k] = s.x;
+  a.v[k] = s.v;
+  a.e[k] = s.e;
+}
+
+// ---------------------------------------------------------------------------------------------
+// S6  moments.  Pass 1: each CTA reduces a contiguous slice of one set (fp64 accumulators,
+// fixed order: per-thread serial, xor-shuffle tree, serial over warps).  Pass 2: one thread
+// per set adds the CTA partials in index order and finalises.  No atomics: reproducible.
+// sums = { N, sum x, sum x^2, sum v, sum v^2, sum e, sum dx, sum dx^2 }, dx = x - x(0).
+// ---------------------------------------------------------------------------------------------
+template <typename Real>
+__global__ void __launch_bounds__(MOM_BLOCK)
+moments_partial_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
+                       const Real* __restrict__ e, const Coef<Real>* __restrict__ coef_table,
+                       uint64_t n_particles, uint64_t traj_base, uint64_t set_stride, uint64_t seed,
+                       uint32_t blocks_per_set, uint32_t slice, double* __restrict__ partial) {
+  const uint32_t set = blockIdx.x / blocks_per_set;
+  const uint32_t blk = blockIdx.x - set * blocks_per_set;
+  const uint64_t r0 = static_cast<uint64_t>(blk) * slice;
+  uint64_t r1 = r0 + slice;
+  if (r1 > n_particles) r1 = n_particles;
+  const Coef<Real> c = coef_table[set];
+  double acc[N_SUMS - 1] = {0, 0, 0, 0, 0, 0, 0};
+  for (uint64_t r = r0 + threadIdx.x; r < r1; r += blockDim.x) {
+    const uint64_t k = static_cast<uint64_t>(set) * n_particles + r;
+    const uint64_t g = traj_base + static_cast<uint64_t>(set) * set_stride + r;
+    const uint4 w = philox_block(seed, g, INIT_BLOCK);
+    const double xi = static_cast<double>(x[k]);
+    const double vi = static_cast<double>(v[k]);
+    const double dx = xi - static_cast<double>(init_x(c, w.x));
+    acc[0] += xi;
+    acc[1] += xi * xi;
+    acc[2] += vi;
+    acc[3] += vi * vi;
+    acc[4] += static_cast<double>(e[k]);
+    acc[5] += dx;
+    acc[6] += dx * dx;
+  }
+  __shared__ double sm[MOM_BLOCK / 32][N_SUMS - 1];
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (int q = 0; q < N_SUMS - 1; ++q) {
+    double t = acc[q];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) t += __shfl_xor_sync(0xffffffffu, t, off);
+    if (lane == 0) sm[warp][q] = t;
+  }
+  __syncthreads();
+  if (threadIdx.x < N_SUMS - 1) {
+    double t = 0;
+    const uint32_t n_warps = (blockDim.x + 31u) >> 5;
+    for (uint32_t wq = 0; wq < n_warps; ++wq) t += sm[wq][threadIdx.x];
+    partial[(static_cast<uint64_t>(blockIdx.x)) * (N_SUMS - 1) + threadIdx.x] = t;
+  }
+}
+
+struct MomentRec {  // mirrors abm_moment (include/abm.h)
+  uint64_t n, step;
+  double mean_x, var_x, mean_v, var_v, mean_e, mean_dx, mean_dx2, mean_x2;
+};
+
+__host__ __device__ inline void finalize_moment(const double* s, uint64_t step, MomentRec* m) {
+  const double N = s[0];
+  m->n = static_cast<uint64_t>(N);
+  m->step = step;
+  const double mx = s[1] / N, mv = s[3] / N;
+  m->mean_x = mx;
+  m->var_x = s[2] / N - mx * mx;
+  m->mean_v = mv;
+  m->var_v = s[4] / N - mv * mv;
+  m->mean_e = s[5] / N;
+  m->mean_dx = s[6] / N;
+  m->mean_dx2 = s[7] / N;
+  m->mean_x2 = s[2] / N;
+}
+
+__global__ void moments_final_kernel(const double* __restrict__ partial, uint32_t n_sets,
+                                     uint32_t blocks_per_set, uint64_t n_particles, uint64_t step,
+                                     double* __restrict__ sums, MomentRec* __restrict__ out) {
+  const uint32_t set = blockIdx.x * blockDim.x + threadIdx.x;
+  if (set >= n_sets) return;
+  double s[N_SUMS];
+  s[0] = static_cast<double>(n_particles);
+  for (int q = 1; q < N_SUMS; ++q) s[q] = 0;
+  const double* p = partial + static_cast<uint64_t>(set) * blocks_per_set * (N_SUMS - 1);
+  for (uint32_t b = 0; b < blocks_per_set; ++b)
+    for (int q = 0; q < N_SUMS - 1; ++q) s[q + 1] += p[static_cast<uint64_t>(b) * (N_SUMS - 1) + q];
+  for (int q = 0; q < N_SUMS; ++q) sums[static_cast<uint64_t>(set) * N_SUMS + q] = s[q];
+  finalize_moment(s, step, &out[set]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Diagnostic: raw Philox blocks of the stream
+// ---------------------------------------------------------------------------------------------
+__global__ void philox_blocks_kernel(uint64_t seed, uint64_t traj_first, uint64_t n_traj,
+                                     uint64_t block_first, uint64_t n_blocks, uint4* out) {
+  const uint64_t t = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (t >= n_traj * n_blocks) return;
+  const uint64_t k = t / n_blocks, j = t - k * n_blocks;
+  out[t] = philox_block(seed, traj_first + k, block_first + j);
+}
+
+}  // namespace abm

@@ -1,0 +1,144 @@
+"""Host-side checks of the C-ABI boundary (no GPU): the library builds, loads, exports every
+function include/abm.h declares, the ctypes mirrors match the C layout, and the error paths
+answer as documented.  No kernel is launched here."""
+import ctypes as C
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "abm.h")
+
+
+@pytest.fixture(scope="module")
+def abm():
+    from paper_1104_2499_b200 import build, binding
+    build.build()
+    binding.lib()
+    return binding
+
+
+def _declared_functions():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(abm_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(abm):
+    names = _declared_functions()
+    assert set(names) == set(abm.EXPORTS), (names, abm.EXPORTS)
+    L = abm.lib()
+    for n in names:
+        assert getattr(L, n) is not None
+    assert L.abm_abi_version() == 1
+
+
+def test_header_is_plain_c_and_layout_matches_ctypes(abm, tmp_path):
+    """Compile a C99 probe against include/abm.h with gcc: the header must be usable from C, and
+    sizeof/offsetof must agree with the ctypes mirrors the tests and bench use."""
+    fields = [f[0] for f in abm.abm_params._fields_]
+    mfields = [f[0] for f in abm.abm_moment._fields_]
+    lines = ['#include <stdio.h>', '#include <stddef.h>', '#include "abm.h"', 'int main(void){',
+             'printf("%zu\\n", sizeof(abm_params));', 'printf("%zu\\n", sizeof(abm_moment));']
+    lines += [f'printf("%zu\\n", offsetof(abm_params, {f}));' for f in fields]
+    lines += [f'printf("%zu\\n", offsetof(abm_moment, {f}));' for f in mfields]
+    lines += ['return 0;}']
+    src = tmp_path / "probe.c"
+    src.write_text("\n".join(lines))
+    exe = tmp_path / "probe"
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"),
+                    "-o", str(exe), str(src)], check=True)
+    vals = [int(v) for v in subprocess.run([str(exe)], check=True, capture_output=True,
+                                           text=True).stdout.split()]
+    assert vals[0] == C.sizeof(abm.abm_params)
+    assert vals[1] == C.sizeof(abm.abm_moment) == 80 == abm.MOMENT_DTYPE.itemsize
+    want = [getattr(abm.abm_params, f).offset for f in fields] + \
+           [getattr(abm.abm_moment, f).offset for f in mfields]
+    assert vals[2:] == want
+
+
+def test_error_paths_without_device(abm):
+    L = abm.lib()
+    h = C.c_void_p()
+    from paper_1104_2499_b200 import workloads as W
+    good = abm.make_params([W.config0().set_params(0)])
+    # argument validation comes first and needs no device
+    assert L.abm_create(None, 16, 1, 1, C.byref(h)) == abm.ABM_EINVAL
+    assert L.abm_create(good, 0, 1, 1, C.byref(h)) == abm.ABM_EINVAL
+    assert L.abm_create(good, 16, 0, 1, C.byref(h)) == abm.ABM_EINVAL
+    assert L.abm_create(good, 16, 1, 1, None) == abm.ABM_EINVAL
+    bad = abm.make_params([W.config0().set_params(0)])
+    bad[0].struct_size = 8
+    assert L.abm_create(bad, 16, 1, 1, C.byref(h)) == abm.ABM_EINVAL
+    for key, val in [("dt", 0.0), ("dt", float("nan")), ("L", -1.0), ("D", -0.1), ("precision", 7),
+                     ("integrator", 2)]:
+        bad = abm.make_params([dict(W.config0().set_params(0), **{key: val})])
+        assert L.abm_create(bad, 16, 1, 1, C.byref(h)) == abm.ABM_EINVAL, key
+    # run-control fields must agree between sets
+    two = abm.make_params([W.config0().set_params(0), dict(W.config0().set_params(0), dt=2e-3)])
+    assert L.abm_create(two, 16, 2, 1, C.byref(h)) == abm.ABM_EINVAL
+    assert h.value is None                                  # *out untouched on error
+    # null / never-created contexts
+    assert L.abm_step(None, 1) == abm.ABM_ESTATE
+    assert L.abm_destroy(None) == abm.ABM_ESTATE
+    assert L.abm_moments(None, None) == abm.ABM_ESTATE
+    assert L.abm_snapshot(None, None, 8) == abm.ABM_ESTATE
+    assert L.abm_philox_blocks(1, 0, 0, 0, 1, None, None) == abm.ABM_EINVAL
+    for code in (0, -1, -2, -3, -4, -99):
+        assert len(L.abm_strerror(code)) > 0
+
+
+def test_no_cpu_fallback(abm):
+    """On a box without a CUDA device a valid abm_create must fail loudly (ABM_ECUDA), never
+    compute on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present; the GPU tests cover the success path")
+    from paper_1104_2499_b200 import workloads as W
+    good = abm.make_params([W.config0().set_params(0)])
+    h = C.c_void_p()
+    assert abm.lib().abm_create(good, 16, 1, 1, C.byref(h)) == abm.ABM_ECUDA
+    with pytest.raises(abm.AbmError):
+        abm.abm_create(good, 16, 1, 1)
+    with pytest.raises(RuntimeError):
+        abm.Ensemble([W.config0().set_params(0)], 16, 1)
+
+
+def test_moments_from_sums_matches_numpy(abm):
+    """abm_moments_from_sums is pure host arithmetic (the shard-combination step)."""
+    rng = np.random.default_rng(3)
+    x, v, e, x0 = rng.normal(2, 3, 500), rng.normal(0, 1, 500), rng.uniform(0, 2, 500), rng.uniform(0, 1, 500)
+    dx = x - x0
+    sums = np.array([[x.size, x.sum(), (x * x).sum(), v.sum(), (v * v).sum(), e.sum(), dx.sum(),
+                      (dx * dx).sum()]])
+    m = abm.abm_moments_from_sums(sums, 77)[0]
+    assert m["n"] == 500 and m["step"] == 77
+    assert m["mean_x"] == pytest.approx(x.mean(), rel=1e-12)
+    assert m["var_x"] == pytest.approx(x.var(), rel=1e-10)
+    assert m["mean_v"] == pytest.approx(v.mean(), rel=1e-10, abs=1e-14)
+    assert m["var_v"] == pytest.approx(v.var(), rel=1e-10)
+    assert m["mean_e"] == pytest.approx(e.mean(), rel=1e-12)
+    assert m["mean_dx"] == pytest.approx(dx.mean(), rel=1e-12)
+    assert m["mean_dx2"] == pytest.approx((dx * dx).mean(), rel=1e-12)
+    assert m["mean_x2"] == pytest.approx((x * x).mean(), rel=1e-12)
+    with pytest.raises(abm.AbmError):
+        abm.abm_moments_from_sums(np.zeros((1, 8)), 0)
+
+
+def test_product_never_imports_oracle():
+    """The oracle is test infrastructure: nothing under the package may import or load it."""
+    pkg = os.path.join(ROOT, "paper_1104_2499_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"import\s+oracle|from\s+oracle|abm_oracle|abo_", txt), (dirpath, f)
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c", ".h")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(import|from)\s+paper_1104_2499_b200", txt, flags=re.M)
+            assert '#include "abm.h"' not in txt and "abm_device" not in txt
