@@ -158,6 +158,7 @@ def run(cfg, seed, x, v, e, step_first, n_steps, traj_first=0, traj_stride=1, th
 
 def moments(x, v, e, x0):
     """-> dict of the eight ensemble moments (population normalisation)."""
+    x, v, e, x0 = (np.ascontiguousarray(a, np.float64) for a in (x, v, e, x0))
     out = np.empty(8, np.float64)
     lib().abo_moments(_dp(x), _dp(v), _dp(e), _dp(x0), x.shape[0], _dp(out))
     names = ["mean_x", "var_x", "mean_v", "var_v", "mean_e", "mean_dx", "mean_dx2", "mean_x2"]

@@ -42,5 +42,24 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+PIPE_RATES_SRC = os.path.join(CSRC, "pipe_rates.cu")
+PIPE_RATES_EXE = os.path.join(PKG, "pipe_rates")
+
+
+def build_pipe_rates(force: bool = False) -> str:
+    """The stand-alone issue-rate diagnostic (csrc/pipe_rates.cu): not needed by the library."""
+    if not force and os.path.exists(PIPE_RATES_EXE) and \
+            os.path.getmtime(PIPE_RATES_EXE) >= os.path.getmtime(PIPE_RATES_SRC):
+        return PIPE_RATES_EXE
+    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+           "-o", PIPE_RATES_EXE, PIPE_RATES_SRC]
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + res.stdout + res.stderr)
+    return PIPE_RATES_EXE
+
+
 if __name__ == "__main__":
     print(build(force=True, verbose="-v" in sys.argv))
+    if "--pipe-rates" in sys.argv:
+        print(build_pipe_rates(force=True))

@@ -90,7 +90,7 @@ Coef<Real> make_coef(const abm_params& p) {
     c.th_o = static_cast<Real>(2.0 * p.phi / p.L);
     c.s2 = static_cast<Real>(std::sqrt(2.0 * p.D * p.dt));  // sigma
   }
-  c.bm_o = static_cast<Real>(two_pi * 0x1p-24);
+  c.bm_o = static_cast<Real>(two_pi * 0x1p-24 - 1.5 * two_pi);
   c.A = static_cast<Real>(p.A);
   c.L = static_cast<Real>(p.L);
   c.v0 = static_cast<Real>(p.v0);

@@ -92,7 +92,7 @@ struct Coef {
   Real s2;             // fp32: -2 sigma^2 ln 2 (so sigma^2 (-2 ln u) = s2 lg2 u); fp64: sigma
   Real A;              // tilt amplitude
   Real L, v0, e0, sv;  // init: x0 = L u, v0, e0, sv = sqrt(D/gamma0)
-  Real bm_o;           // fp32: 2 pi 2^-24, the half-ulp offset of the Box-Muller angle
+  Real bm_o;           // fp32: 2 pi 2^-24 - 3 pi, offset of the Box-Muller angle (see S2)
   Real pad[2];
 };
 static_assert(sizeof(Coef<float>) == 80, "Coef<float> layout");
@@ -104,13 +104,19 @@ struct State {
 };
 
 // ---------------------------------------------------------------------------------------------
-// S2  Box-Muller on a word pair -> (rho, cos, sin) with rho = sigma sqrt(-2 ln u1) so that
+// S2  Box-Muller on a word pair -> (rho, cs, sn) with rho = sigma sqrt(-2 ln u1) and
 // sigma z_even = rho cos(2 pi u2), sigma z_odd = rho sin(2 pi u2).
 // fp32 uniform map ((w >> 9) + 0.5) 2^-23, built exactly as m - (1 - 2^-24) with
 // m = as_float((w >> 9) + 0x3f800000) in [1, 2).
+//
+// fp32: the angle handed to MUFU is 2 pi u2 - pi, in [-pi, pi), where one FMA rounds to at most
+// 2^-23 rad (four times finer than on [2 pi, 4 pi)); that half turn flips the sign of both
+// functions, so Normal2f carries cs = -cos(2 pi u2), sn = -sin(2 pi u2) and NEGATED = true tells
+// the caller to use -rho (an operand modifier of the consuming FMA, no instruction).
 // ---------------------------------------------------------------------------------------------
 struct Normal2f {
   float rho, cs, sn;
+  static constexpr bool NEGATED = true;
 };
 
 __device__ __forceinline__ float uniform_f32(uint32_t w) {
@@ -123,7 +129,7 @@ __device__ __forceinline__ Normal2f box_muller_f32(uint32_t wa, uint32_t wb, flo
   Normal2f o;
   const float u1 = uniform_f32(wa);
   o.rho = fast_sqrt(__fmul_rn(fast_lg2(u1), s2));
-  // angle 2 pi u2 = 2 pi (m - 1 + 2^-24), m in [1, 2): the "- 2 pi" is a whole turn, so one FMA
+  // 2 pi u2 - pi = 2 pi (m - 1 + 2^-24) - pi = 2 pi m + bm_o,  bm_o = 2 pi 2^-24 - 3 pi
   const float m2 = __uint_as_float((wb >> 9) + 0x3f800000u);
   const float ang = __fmaf_rn(m2, 6.283185307179586f, bm_o);
   o.cs = fast_cos(ang);
@@ -133,6 +139,7 @@ __device__ __forceinline__ Normal2f box_muller_f32(uint32_t wa, uint32_t wb, flo
 
 struct Normal2d {
   double rho, cs, sn;
+  static constexpr bool NEGATED = false;
 };
 
 __device__ __forceinline__ double uniform_f64(uint32_t w) {

@@ -124,12 +124,14 @@ template <typename Real>
 struct Noise4;
 template <>
 struct Noise4<float> {
+  static constexpr float SIGN = Normal2f::NEGATED ? -1.0f : 1.0f;
   Normal2f a, b;
   __device__ __forceinline__ Noise4(const uint4& w, const Coef<float>& k)
       : a(box_muller_f32(w.x, w.y, k.s2, k.bm_o)), b(box_muller_f32(w.z, w.w, k.s2, k.bm_o)) {}
 };
 template <>
 struct Noise4<double> {
+  static constexpr double SIGN = Normal2d::NEGATED ? -1.0 : 1.0;
   Normal2d a, b;
   __device__ __forceinline__ Noise4(const uint4& w, const Coef<double>& k)
       : a(box_muller_f64(w.x, w.y, k.s2)), b(box_muller_f64(w.z, w.w, k.s2)) {}
@@ -200,10 +202,11 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
           if (INTEG == 1) t4 = tl[4];
           tl += 4;
         }
-        one_step<Real, INTEG, TILT>(s, cf, z.a.rho, z.a.cs, t0, t1);
-        one_step<Real, INTEG, TILT>(s, cf, z.a.rho, z.a.sn, t1, t2);
-        one_step<Real, INTEG, TILT>(s, cf, z.b.rho, z.b.cs, t2, t3);
-        one_step<Real, INTEG, TILT>(s, cf, z.b.rho, z.b.sn, t3, t4);
+        const Real ra = Noise4<Real>::SIGN * z.a.rho, rb = Noise4<Real>::SIGN * z.b.rho;
+        one_step<Real, INTEG, TILT>(s, cf, ra, z.a.cs, t0, t1);
+        one_step<Real, INTEG, TILT>(s, cf, ra, z.a.sn, t1, t2);
+        one_step<Real, INTEG, TILT>(s, cf, rb, z.b.cs, t2, t3);
+        one_step<Real, INTEG, TILT>(s, cf, rb, z.b.sn, t3, t4);
       } while (++b_lo != b_end);
       n += static_cast<uint64_t>(nb) << 2;
     } else {
@@ -211,7 +214,7 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
       const uint4 w = philox_block(a.seed, id.global, n >> 2);
       const Noise4<Real> z(w, cf);
       const bool second = (n >> 1) & 1u;
-      const Real rho = second ? z.b.rho : z.a.rho;
+      const Real rho = Noise4<Real>::SIGN * (second ? z.b.rho : z.a.rho);
       const Real cs = (n & 1u) ? (second ? z.b.sn : z.a.sn) : (second ? z.b.cs : z.a.cs);
       Real t0 = 0, t1 = 0;
       if (TILT) {

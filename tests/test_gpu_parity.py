@@ -73,12 +73,19 @@ def test_normals_consumed_by_the_step_kernel(abm, oracle):
     dt = 2.0**-10
     p = dict(W.DEFAULTS, A1=0.0, A2=0.0, d=0.0, q=0.0, c=0.0, gamma0=1.0 / dt, dt=dt, D=0.5 / dt)
     N, seed = 4096, 31337
+    # Error budget of one normal z = rho * trig(angle) built from MUFU approximations (PTX ISA:
+    # lg2.approx max abs error 2^-22; sin/cos.approx ~2^-21 abs on [-pi, pi]; sqrt.approx ~1 ulp):
+    #   rho^2 = 2 ln2 * (-lg2 u1)  =>  |d rho| <= ln2 * 2^-22 / rho   (dominates for small rho)
+    #   angle: one FMA rounding on [-pi, pi) + range-scale multiply ~4e-7 rad, MUFU ~5e-7
+    #   => |dz| <= 1.7e-7 / rho + 1.0e-6 * (1 + rho)
     with abm.Ensemble([p], N, seed) as ens:
         for n in range(8):
             ens.step(1)
             z = ens.state()[:, 1]                       # sigma = sqrt(2 D dt) = 1
-            want = oracle.normals(seed, 0, N, n, 1, 0)[:, 0]
-            assert np.abs(z - want).max() < 4e-6, n     # MUFU lg2/sqrt/sin/cos absolute error
+            pair = oracle.normals(seed, 0, N, n & ~1, 2, 0)
+            want, rho = pair[:, n & 1], np.hypot(pair[:, 0], pair[:, 1])
+            bound = 1.7e-7 / np.maximum(rho, 1e-4) + 1.0e-6 * (1.0 + rho)
+            assert np.all(np.abs(z - want) <= bound), (n, np.max(np.abs(z - want) / bound))
             assert np.abs(z - want).mean() < 4e-7
 
 
@@ -356,10 +363,14 @@ def test_gpu_ou_variance_exact_recursion(abm):
 
 @pytest.mark.parametrize("precision", [0, 1])
 def test_gpu_depot_stationary_speed(abm, precision):
+    """Pin P5 on the GPU.  In fp32 the recursion stalls once an increment drops under half an ulp
+    of the state (the paper's warning about adding small numbers to large ones):
+    dt |a_e| < ulp(e)/2 = 6e-8 and dt |a_v| < ulp(v)/2 = 3e-8 leave |e - 1| <~ 3e-5 and
+    |q - c e - d e v^2| <~ 6e-5, i.e. v^2 within ~1e-4 of q/gamma0 - c/d.  fp64 reaches 1e-10."""
     p = dict(W.DEFAULTS, A1=0.0, A2=0.0, D=0.0, v0=0.05, precision=precision)
     with abm.Ensemble([p], 64, 1) as ens:
         ens.step(200_000)
         st = ens.state()
-    tol = 1e-5 if precision == 0 else 1e-10
+    tol = 1e-4 if precision == 0 else 1e-10
     assert st[:, 1]**2 == pytest.approx(1.0 / 1.0 - 0.1 / 1.0, rel=tol)
     assert st[:, 2] == pytest.approx(1.0, rel=tol)
