@@ -62,6 +62,16 @@ typedef enum abm_status {
 enum { ABM_FP32 = 0, ABM_FP64 = 1 };               /* abm_params.precision  */
 enum { ABM_EULER_MARUYAMA = 0, ABM_HEUN = 1 };     /* abm_params.integrator */
 enum { ABM_INIT_V_CONST = 0, ABM_INIT_V_THERMAL = 1 }; /* abm_params.init_v */
+/* abm_params.accuracy -- "precise vs fast intrinsics chosen against the stated tolerance"
+ * (BASELINE.json north_star (b): fp32 state within 1e-5 of the fp64 oracle after 100 steps).
+ *   FAST     angle 2 pi (x + phi) / L handed to MUFU.COS as is; x' = x + dt v in one FMA.
+ *   PRECISE  whole periods removed from x exactly before the cosine, and x carried as an
+ *            unevaluated sum of two floats (compensated x update): +6 FP32 instructions per
+ *            Euler-Maruyama step, +9 per Heun step; one more float of state per trajectory.
+ *   AUTO     PRECISE if dt (2 pi / L)^2 (|A1| + 4 |A2|) > 0.15 for any set, else FAST
+ *            (configs[0-2]: 0.079 -> FAST; config[3]: 0.39 -> PRECISE).
+ * Ignored in fp64.  Both modes consume the same random stream. */
+enum { ABM_ACCURACY_AUTO = 0, ABM_ACCURACY_FAST = 1, ABM_ACCURACY_PRECISE = 2 };
 
 typedef struct abm_ctx abm_ctx; /* opaque, owned by the library */
 
@@ -74,7 +84,7 @@ typedef struct abm_params {
   uint32_t init_v;         /* RC  v(0) = v0, or v(0) ~ N(0, D/gamma0) from the init block      */
   uint32_t snapshot_every; /* RC  K: abm_step rewrites the bound snapshot buffer after every
                                   global step count that is a multiple of K; 0 = never         */
-  uint32_t reserved0;
+  uint32_t accuracy;       /* RC  fp32 only: ABM_ACCURACY_AUTO | _FAST | _PRECISE (see below)      */
   double dt;               /* RC  time step                                                    */
   double gamma0, q, c, d, D; /*   Eqs. 1-2                                                     */
   double F0;               /*     constant load force, +F0 as printed in Eq. 2   */
@@ -137,6 +147,9 @@ int abm_moments_from_sums(const double* sums, uint32_t n_param_sets, uint64_t st
 
 /* Global step count reached so far. */
 int abm_get_step(const abm_ctx* ctx, uint64_t* out_step);
+
+/* The fp32 accuracy mode in effect (ABM_ACCURACY_FAST or _PRECISE; AUTO is resolved at create). */
+int abm_get_accuracy(const abm_ctx* ctx, uint32_t* out_mode);
 
 /* Wait for the context's stream and free everything the library owns. */
 int abm_destroy(abm_ctx* ctx);

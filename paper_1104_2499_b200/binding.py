@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_PKG, "libabm_b200.so")
 ABM_OK, ABM_EINVAL, ABM_ENOMEM, ABM_ECUDA, ABM_ESTATE = 0, -1, -2, -3, -4
 ABM_FP32, ABM_FP64 = 0, 1
 ABM_EULER_MARUYAMA, ABM_HEUN = 0, 1
+ABM_ACCURACY_AUTO, ABM_ACCURACY_FAST, ABM_ACCURACY_PRECISE = 0, 1, 2
 ABM_N_SUMS = 8
 
 
@@ -23,7 +24,7 @@ class abm_params(C.Structure):
     """Mirror of `abm_params` (include/abm.h)."""
     _fields_ = [
         ("struct_size", C.c_uint32), ("precision", C.c_uint32), ("integrator", C.c_uint32),
-        ("init_v", C.c_uint32), ("snapshot_every", C.c_uint32), ("reserved0", C.c_uint32),
+        ("init_v", C.c_uint32), ("snapshot_every", C.c_uint32), ("accuracy", C.c_uint32),
         ("dt", C.c_double), ("gamma0", C.c_double), ("q", C.c_double), ("c", C.c_double),
         ("d", C.c_double), ("D", C.c_double), ("F0", C.c_double), ("A", C.c_double),
         ("omega", C.c_double), ("L", C.c_double), ("A1", C.c_double), ("A2", C.c_double),
@@ -45,7 +46,7 @@ MOMENT_DTYPE = np.dtype([("n", "<u8"), ("step", "<u8"), ("mean_x", "<f8"), ("var
                          ("mean_dx", "<f8"), ("mean_dx2", "<f8"), ("mean_x2", "<f8")])
 
 EXPORTS = ["abm_create", "abm_step", "abm_snapshot", "abm_snapshot_host", "abm_moments",
-           "abm_moment_sums", "abm_moments_from_sums", "abm_get_step", "abm_destroy",
+           "abm_moment_sums", "abm_moments_from_sums", "abm_get_step", "abm_get_accuracy", "abm_destroy",
            "abm_philox_blocks", "abm_strerror", "abm_abi_version"]
 
 _lib = None
@@ -75,6 +76,7 @@ def lib():
         L.abm_moment_sums.argtypes = [vp, vp]
         L.abm_moments_from_sums.argtypes = [vp, u32, u64, vp]
         L.abm_get_step.argtypes = [vp, C.POINTER(u64)]
+        L.abm_get_accuracy.argtypes = [vp, C.POINTER(u32)]
         L.abm_destroy.argtypes = [vp]
         L.abm_philox_blocks.argtypes = [u64, u64, u64, u64, u64, vp, vp]
         for n in EXPORTS[:-2]:
@@ -87,7 +89,7 @@ def lib():
     return _lib
 
 
-_PARAM_KEYS = ["precision", "integrator", "init_v", "snapshot_every", "dt", "gamma0", "q", "c", "d",
+_PARAM_KEYS = ["precision", "integrator", "init_v", "snapshot_every", "accuracy", "dt", "gamma0", "q", "c", "d",
                "D", "F0", "A", "omega", "L", "A1", "A2", "phi", "v0", "e0", "traj_base",
                "traj_set_stride"]
 
@@ -158,6 +160,12 @@ def abm_get_step(ctx):
     return n.value
 
 
+def abm_get_accuracy(ctx):
+    m = C.c_uint32()
+    _check("abm_get_accuracy", lib().abm_get_accuracy(ctx, C.byref(m)))
+    return m.value
+
+
 def abm_destroy(ctx):
     _check("abm_destroy", lib().abm_destroy(ctx))
 
@@ -179,7 +187,7 @@ class Ensemble:
     """
 
     def __init__(self, param_sets, n_particles, seed, snapshot_every=0, stream=None,
-                 traj_base=0, traj_set_stride=0):
+                 traj_base=0, traj_set_stride=0, accuracy=ABM_ACCURACY_AUTO):
         import torch
         self._torch = torch
         if not torch.cuda.is_available():
@@ -193,7 +201,7 @@ class Ensemble:
         else:
             params = make_params(param_sets, stream=self.stream.cuda_stream,
                                  snapshot_every=snapshot_every, traj_base=traj_base,
-                                 traj_set_stride=traj_set_stride)
+                                 traj_set_stride=traj_set_stride, accuracy=accuracy)
         self.fp64 = int(params[0].precision) == 1
         self.ctx = abm_create(params, n_particles, self.n_sets, seed)
         self.frame = None
@@ -227,6 +235,10 @@ class Ensemble:
         host = np.empty((self.n_traj, cols), np.float64 if self.fp64 else np.float32)
         abm_snapshot_host(self.ctx, host, cols * item)
         return host[:, :3].astype(np.float64)
+
+    @property
+    def accuracy(self):
+        return abm_get_accuracy(self.ctx)
 
     @property
     def step_count(self):

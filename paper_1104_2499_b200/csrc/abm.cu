@@ -35,10 +35,12 @@ struct abm_ctx {
   uint32_t precision, integrator, init_v, snap_every;
   uint32_t n_sets;
   bool tilt;
+  bool precise;         // fp32 accuracy mode resolved at create (include/abm.h, abm_params.accuracy)
   uint64_t n_particles, n_traj, seed, step, traj_base, set_stride;
   double dt, omega;
   size_t real_size;
   void *x, *v, *e;      // state, SoA, Real[n_traj]
+  void* xl;             // low part of x, float[n_traj] (precise fp32 mode only)
   void* coef_table;     // Coef<Real>[n_sets]
   void* tilt_table;     // Real[TILT_CHUNK + 1]
   double* partial;      // [n_sets * blocks_per_set][7]
@@ -91,12 +93,24 @@ Coef<Real> make_coef(const abm_params& p) {
     c.s2 = static_cast<Real>(std::sqrt(2.0 * p.D * p.dt));  // sigma
   }
   c.bm_o = static_cast<Real>(two_pi * 0x1p-24 - 1.5 * two_pi);
+  c.inv_L = static_cast<Real>(1.0 / p.L);
   c.A = static_cast<Real>(p.A);
   c.L = static_cast<Real>(p.L);
   c.v0 = static_cast<Real>(p.v0);
   c.e0 = static_cast<Real>(p.e0);
   c.sv = static_cast<Real>(p.init_v ? std::sqrt(p.D / p.gamma0) : 0.0);
   return c;
+}
+
+// dt * max|U''(x)| <= dt (2 pi / L)^2 (|A1| + 4 |A2|): the factor by which one step turns a
+// position error into a velocity error.  The 100-step fp32-vs-fp64 deviation grows in proportion
+// to it (3.6e-6 at 0.079 = configs[0-2], 8e-6..1e-5 at 0.39 =
+// config[3], against the 1e-5 of BASELINE.json), so ABM_ACCURACY_AUTO switches to the precise
+// kernels above PRECISE_ABOVE.
+constexpr double PRECISE_ABOVE = 0.15;
+double stiffness(const abm_params& p) {
+  const double g = 6.283185307179586476925286766559 / p.L;
+  return p.dt * g * g * (std::fabs(p.A1) + 4.0 * std::fabs(p.A2));
 }
 
 bool finite_all(const abm_params& p) {
@@ -111,13 +125,14 @@ int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets) {
   if (!params || n_particles == 0 || n_sets == 0) return ABM_EINVAL;
   const abm_params& p0 = params[0];
   if (p0.struct_size != sizeof(abm_params)) return ABM_EINVAL;
-  if (p0.precision > ABM_FP64 || p0.integrator > ABM_HEUN || p0.init_v > ABM_INIT_V_THERMAL)
+  if (p0.precision > ABM_FP64 || p0.integrator > ABM_HEUN || p0.init_v > ABM_INIT_V_THERMAL ||
+      p0.accuracy > ABM_ACCURACY_PRECISE)
     return ABM_EINVAL;
   for (uint32_t s = 0; s < n_sets; ++s) {
     const abm_params& p = params[s];
     if (p.struct_size != sizeof(abm_params)) return ABM_EINVAL;
     if (p.precision != p0.precision || p.integrator != p0.integrator || p.init_v != p0.init_v ||
-        p.snapshot_every != p0.snapshot_every || p.dt != p0.dt || p.omega != p0.omega ||
+        p.accuracy != p0.accuracy || p.snapshot_every != p0.snapshot_every || p.dt != p0.dt || p.omega != p0.omega ||
         p.traj_base != p0.traj_base || p.traj_set_stride != p0.traj_set_stride ||
         p.stream != p0.stream)
       return ABM_EINVAL;
@@ -136,6 +151,7 @@ void free_all(abm_ctx* c) {
   cudaFree(c->x);
   cudaFree(c->v);
   cudaFree(c->e);
+  cudaFree(c->xl);
   cudaFree(c->coef_table);
   cudaFree(c->tilt_table);
   cudaFree(c->partial);
@@ -161,14 +177,22 @@ int upload_coefs_and_init(abm_ctx* c, const abm_params* params) {
   return ABM_OK;
 }
 
-template <typename Real, int INTEG, bool TILT>
-cudaError_t launch_step_u(const abm_ctx* c, const StepArgs<Real>& a) {
+template <typename Real, int INTEG, bool TILT, bool PRECISE>
+cudaError_t launch_step_p(const abm_ctx* c, const StepArgs<Real>& a) {
   const uint32_t grid = static_cast<uint32_t>((c->n_traj + STEP_BLOCK - 1) / STEP_BLOCK);
   if (c->n_sets == 1)
-    step_kernel<Real, INTEG, TILT, true><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+    step_kernel<Real, INTEG, TILT, true, PRECISE><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
   else
-    step_kernel<Real, INTEG, TILT, false><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+    step_kernel<Real, INTEG, TILT, false, PRECISE><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
   return cudaGetLastError();
+}
+
+template <typename Real, int INTEG, bool TILT>
+cudaError_t launch_step_u(const abm_ctx* c, const StepArgs<Real>& a) {
+  if constexpr (sizeof(Real) == 4) {  // the accuracy modes exist in fp32 only
+    if (c->precise) return launch_step_p<Real, INTEG, TILT, true>(c, a);
+  }
+  return launch_step_p<Real, INTEG, TILT, false>(c, a);
 }
 
 template <typename Real>
@@ -191,6 +215,7 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
   a.x = static_cast<Real*>(c->x);
   a.v = static_cast<Real*>(c->v);
   a.e = static_cast<Real*>(c->e);
+  a.xl = static_cast<Real*>(c->xl);
   a.coef_table = static_cast<const Coef<Real>*>(c->coef_table);
   a.tilt = static_cast<const Real*>(c->tilt_table);
   a.snap = c->snap;
@@ -295,6 +320,13 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   for (uint32_t s = 0; s < n_param_sets; ++s)
     if (params[s].A != 0.0) c->tilt = true;
   c->real_size = c->precision == ABM_FP32 ? 4 : 8;
+  c->precise = false;
+  if (c->precision == ABM_FP32) {
+    if (p0.accuracy == ABM_ACCURACY_PRECISE) c->precise = true;
+    if (p0.accuracy == ABM_ACCURACY_AUTO)
+      for (uint32_t s = 0; s < n_param_sets; ++s)
+        if (stiffness(params[s]) > PRECISE_ABOVE) c->precise = true;
+  }
   c->coef0_f = make_coef<float>(p0);
   c->coef0_d = make_coef<double>(p0);
 
@@ -328,12 +360,15 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   };
   const size_t state_bytes = c->real_size * c->n_traj;
   if (!alloc(&c->x, state_bytes) || !alloc(&c->v, state_bytes) || !alloc(&c->e, state_bytes) ||
+      (c->precise && !alloc(&c->xl, state_bytes)) ||
       !alloc(reinterpret_cast<void**>(&c->partial),
              sizeof(double) * (N_SUMS - 1) * bps * n_param_sets) ||
       !alloc(reinterpret_cast<void**>(&c->sums), sizeof(double) * N_SUMS * n_param_sets) ||
       !alloc(reinterpret_cast<void**>(&c->moments), sizeof(MomentRec) * n_param_sets) ||
       (c->tilt && !alloc(&c->tilt_table, c->real_size * (TILT_CHUNK + 1))))
     return fail(rc);
+  if (c->precise && cudaMemsetAsync(c->xl, 0, state_bytes, c->stream) != cudaSuccess)
+    return fail(ABM_ECUDA);
   rc = c->precision == ABM_FP32 ? upload_coefs_and_init<float>(c, params)
                                 : upload_coefs_and_init<double>(c, params);
   if (rc != ABM_OK) return fail(rc);
@@ -428,6 +463,13 @@ int abm_get_step(const abm_ctx* c, uint64_t* out_step) {
   return ABM_OK;
 }
 
+int abm_get_accuracy(const abm_ctx* c, uint32_t* out_mode) {
+  if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
+  if (!out_mode) return ABM_EINVAL;
+  *out_mode = c->precise ? ABM_ACCURACY_PRECISE : ABM_ACCURACY_FAST;
+  return ABM_OK;
+}
+
 int abm_destroy(abm_ctx* c) {
   if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
   cudaStreamSynchronize(c->stream);
@@ -460,6 +502,6 @@ const char* abm_strerror(int status) {
   }
 }
 
-uint32_t abm_abi_version(void) { return 1; }
+uint32_t abm_abi_version(void) { return 2; }
 
 }  // extern "C"

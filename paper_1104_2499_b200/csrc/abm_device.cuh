@@ -93,7 +93,8 @@ struct Coef {
   Real A;              // tilt amplitude
   Real L, v0, e0, sv;  // init: x0 = L u, v0, e0, sv = sqrt(D/gamma0)
   Real bm_o;           // fp32: 2 pi 2^-24 - 3 pi, offset of the Box-Muller angle (see S2)
-  Real pad[2];
+  Real inv_L;          // 1 / L (precise fp32 mode: exact reduction of x modulo L)
+  Real pad;
 };
 static_assert(sizeof(Coef<float>) == 80, "Coef<float> layout");
 static_assert(sizeof(Coef<double>) == 160, "Coef<double> layout");
@@ -101,6 +102,7 @@ static_assert(sizeof(Coef<double>) == 160, "Coef<double> layout");
 template <typename Real>
 struct State {
   Real x, v, e;
+  Real xl;  // precise fp32 mode only: running rounding error of x (x + xl is the position)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -156,11 +158,25 @@ __device__ __forceinline__ Normal2d box_muller_f64(uint32_t wa, uint32_t wb, dou
 // ---------------------------------------------------------------------------------------------
 // S3  force  -U'(x) + F0 (+ tilt folded into k0t by the caller):  one cosine per evaluation,
 // cos 2th = 2 cos^2 th - 1  (Eq. 3).
+//
+// fp32, fast mode: th = th_s x + th_o in radians goes straight to MUFU.COS (through the
+// range-scale multiply ptxas puts in front of it): two roundings at the magnitude of th, up to
+// ~2.4e-6 rad for |x| ~ 3 L.  Precise mode first removes whole periods from x EXACTLY
+// (k = rint(x / L) by the 1.5 * 2^23 trick, xr = x - k L is exact in one FMA), so the angle is
+// rounded at magnitude <= pi (+ phase): ~3e-7 rad.  Three more FP32 instructions per evaluation.
 // ---------------------------------------------------------------------------------------------
+template <bool PRECISE>
 __device__ __forceinline__ float force(const Coef<float>& k, float x, float k0t) {
-  const float c = fast_cos(__fmaf_rn(x, k.th_s, k.th_o));
+  float xr = x;
+  if (PRECISE) {
+    const float magic = 12582912.0f;  // 1.5 * 2^23: adding it rounds to an integer
+    const float n = __fadd_rn(__fmaf_rn(x, k.inv_L, magic), -magic);
+    xr = __fmaf_rn(-n, k.L, x);
+  }
+  const float c = fast_cos(__fmaf_rn(xr, k.th_s, k.th_o));
   return __fmaf_rn(__fmaf_rn(k.k2, c, k.k1), c, k0t);
 }
+template <bool PRECISE>
 __device__ __forceinline__ double force(const Coef<double>& k, double x, double k0t) {
   const double c = cospi(__fma_rn(x, k.th_s, k.th_o));
   return __fma_rn(__fma_rn(k.k2, c, k.k1), c, k0t);
@@ -183,34 +199,51 @@ __device__ __forceinline__ double add_(double a, double b) { return __dadd_rn(a,
 // The increments are added to the state unscaled (no pre-multiplied (1 - gamma0 dt) factors):
 // a rounded factor next to 1 would bias every step in the same direction.
 // ---------------------------------------------------------------------------------------------
-template <typename Real>
+//
+// Precise fp32 mode: the rounding of x' = x + dt v is what limits the
+// 100-step agreement with the fp64 oracle (the error random-walks in x and is amplified by
+// dt U''), so x is carried as an unevaluated sum x + xl (Fast2Sum of the increment; xl feeds the
+// next increment).  Three more FP32 instructions per step.
+template <bool PRECISE, typename Real>
+__device__ __forceinline__ void advance_x(State<Real>& s, Real h, Real w) {  // x += h * w
+  if (PRECISE) {
+    const Real inc = fma_(h, w, s.xl);
+    const Real xn = add_(s.x, inc);
+    s.xl = add_(inc, -add_(xn, -s.x));
+    s.x = xn;
+  } else {
+    s.x = fma_(h, w, s.x);
+  }
+}
+
+template <bool PRECISE, typename Real>
 __device__ __forceinline__ void em_step(State<Real>& s, const Coef<Real>& k, Real k0t, Real rho,
                                         Real cs) {
-  const Real f = force(k, s.x, k0t);
+  const Real f = force<PRECISE>(k, s.x, k0t);
   const Real av = fma_(fma_(k.d, s.e, -k.gamma0), s.v, f);
   const Real ae = fma_(-s.e, fma_(k.d, mul_(s.v, s.v), k.c), k.q);
-  s.x = fma_(k.dt, s.v, s.x);
+  advance_x<PRECISE>(s, k.dt, s.v);
   s.v = fma_(rho, cs, fma_(k.dt, av, s.v));
   s.e = fma_(k.dt, ae, s.e);
 }
 
 // Stochastic Heun: predictor = EM step with the full noise increment; corrector averages the
 // drift at (X, t_n) and (X~, t_{n+1}); the same sigma z in both (reading G16).
-template <typename Real>
+template <bool PRECISE, typename Real>
 __device__ __forceinline__ void heun_step(State<Real>& s, const Coef<Real>& k, Real k0t, Real k0t1,
                                           Real rho, Real cs) {
   const Real sz = mul_(rho, cs);
-  const Real f1 = force(k, s.x, k0t);
+  const Real f1 = force<PRECISE>(k, s.x, k0t);
   const Real av1 = fma_(fma_(k.d, s.e, -k.gamma0), s.v, f1);
   const Real ae1 = fma_(-s.e, fma_(k.d, mul_(s.v, s.v), k.c), k.q);
   const Real xp = fma_(k.dt, s.v, s.x);
-  const Real vp = add_(fma_(k.dt, av1, s.v), sz);
+  const Real vp = add_(s.v, fma_(k.dt, av1, sz));
   const Real ep = fma_(k.dt, ae1, s.e);
-  const Real f2 = force(k, xp, k0t1);
+  const Real f2 = force<PRECISE>(k, xp, k0t1);
   const Real av2 = fma_(fma_(k.d, ep, -k.gamma0), vp, f2);
   const Real ae2 = fma_(-ep, fma_(k.d, mul_(vp, vp), k.c), k.q);
-  s.x = fma_(k.hdt, add_(s.v, vp), s.x);
-  s.v = add_(fma_(k.hdt, add_(av1, av2), s.v), sz);
+  advance_x<PRECISE>(s, k.hdt, add_(s.v, vp));
+  s.v = add_(s.v, fma_(k.hdt, add_(av1, av2), sz));  // one rounding at the magnitude of v
   s.e = fma_(k.hdt, add_(ae1, ae2), s.e);
 }
 

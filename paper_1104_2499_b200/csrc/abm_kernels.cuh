@@ -16,6 +16,7 @@ struct StepArgs {
   Real* x;
   Real* v;
   Real* e;
+  Real* xl;                      // low part of x (used when PRECISE; else nullptr)
   const Coef<Real>* coef_table;  // [n_sets] (used when !UNIFORM)
   const Real* tilt;              // tilt[j] = cos(omega (tilt_base + j) dt) (used when TILT)
   void* snap;                    // bound snapshot buffer or nullptr
@@ -80,7 +81,7 @@ __global__ void snapshot_kernel(const Real* __restrict__ x, const Real* __restri
                                 uint32_t stride) {
   const uint64_t k = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (k >= n_traj) return;
-  State<Real> s{x[k], v[k], e[k]};
+  State<Real> s{x[k], v[k], e[k], Real(0)};
   store_snapshot(snap, stride, k, s);
 }
 
@@ -137,19 +138,19 @@ struct Noise4<double> {
       : a(box_muller_f64(w.x, w.y, k.s2)), b(box_muller_f64(w.z, w.w, k.s2)) {}
 };
 
-template <typename Real, int INTEG, bool TILT>
+template <typename Real, int INTEG, bool TILT, bool PRECISE>
 __device__ __forceinline__ void one_step(State<Real>& s, const Coef<Real>& k, Real rho, Real cs,
                                          Real t0, Real t1) {
   const Real k0t = TILT ? fma_(k.A, t0, k.k0) : k.k0;
   if (INTEG == 0) {
-    em_step(s, k, k0t, rho, cs);
+    em_step<PRECISE>(s, k, k0t, rho, cs);
   } else {
     const Real k0t1 = TILT ? fma_(k.A, t1, k.k0) : k.k0;
-    heun_step(s, k, k0t, k0t1, rho, cs);
+    heun_step<PRECISE>(s, k, k0t, k0t1, rho, cs);
   }
 }
 
-template <typename Real, int INTEG, bool TILT, bool UNIFORM>
+template <typename Real, int INTEG, bool TILT, bool UNIFORM, bool PRECISE>
 __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const __grid_constant__ StepArgs<Real> a) {
   const uint64_t k = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
   if (k >= a.n_traj) return;
@@ -168,7 +169,7 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
     cf.bm_o = g->bm_o;
   }
 
-  State<Real> s{a.x[k], a.v[k], a.e[k]};
+  State<Real> s{a.x[k], a.v[k], a.e[k], PRECISE ? a.xl[k] : Real(0)};
 
   uint64_t n = a.step0;
   const uint64_t n_end = a.step0 + a.n_steps;
@@ -176,8 +177,12 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
   uint64_t next_snap = ~0ull;
   if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
 
+  // Frames fall on Philox-block boundaries when K is a multiple of 4 (n is a multiple of 4 on the
+  // fast path): they are then stored from inside the block loop and the software pipeline below
+  // runs through them.  Otherwise a run of whole blocks ends at the next frame.
+  const bool snap_aligned = (K & 3u) == 0;
   while (n < n_end) {
-    const uint64_t lim = next_snap < n_end ? next_snap : n_end;
+    const uint64_t lim = (snap_aligned || next_snap > n_end) ? n_end : next_snap;
     if ((n & 3u) == 0 && lim - n >= 4) {
       // ---- fast path: whole Philox blocks, four steps each ----
       uint64_t b = n >> 2;
@@ -188,27 +193,49 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
       const uint32_t b_hi = static_cast<uint32_t>(b >> 32);
       uint32_t b_lo = static_cast<uint32_t>(b);
       const Real* tl = TILT ? a.tilt + (n - a.tilt_base) : nullptr;
-      const uint32_t b_end = b_lo + nb;  // may wrap to 0: the loop runs until equality
-#pragma unroll 1
+      uint64_t to_snap = (K && snap_aligned) ? (next_snap - n) >> 2 : ~0ull;  // blocks to the frame
+      uint32_t left = nb;
+      // Software pipeline: the Philox block of the NEXT four steps is computed next to the
+      // floating-point work of the current four, so every warp issues a steady mix of
+      // IMAD.WIDE / LOP3 (fmaheavy + alu pipes) and FFMA / MUFU (fma + xu pipes) instead of an
+      // integer phase followed by a floating-point phase.  The block after the last one of this
+      // run is computed and dropped (its counter may wrap: harmless).
+      uint4 w = philox4x32_10(b_lo, b_hi, static_cast<uint32_t>(id.global),
+                              static_cast<uint32_t>(id.global >> 32),
+                              static_cast<uint32_t>(a.seed), static_cast<uint32_t>(a.seed >> 32));
       do {
-        const uint4 w = philox4x32_10(b_lo, b_hi, static_cast<uint32_t>(id.global),
-                                      static_cast<uint32_t>(id.global >> 32),
-                                      static_cast<uint32_t>(a.seed),
-                                      static_cast<uint32_t>(a.seed >> 32));
-        const Noise4<Real> z(w, cf);
-        Real t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0;
-        if (TILT) {
-          t0 = tl[0]; t1 = tl[1]; t2 = tl[2]; t3 = tl[3];
-          if (INTEG == 1) t4 = tl[4];
-          tl += 4;
+        const uint32_t seg = left < to_snap ? left : static_cast<uint32_t>(to_snap);  // >= 1
+        const uint32_t seg_end = b_lo + seg;  // may wrap to 0: the loop runs until equality
+#pragma unroll 1
+        do {
+          const uint4 w_next = philox4x32_10(b_lo + 1u, b_hi, static_cast<uint32_t>(id.global),
+                                             static_cast<uint32_t>(id.global >> 32),
+                                             static_cast<uint32_t>(a.seed),
+                                             static_cast<uint32_t>(a.seed >> 32));
+          const Noise4<Real> z(w, cf);
+          w = w_next;
+          Real t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0;
+          if (TILT) {
+            t0 = tl[0]; t1 = tl[1]; t2 = tl[2]; t3 = tl[3];
+            if (INTEG == 1) t4 = tl[4];
+            tl += 4;
+          }
+          const Real ra = Noise4<Real>::SIGN * z.a.rho, rb = Noise4<Real>::SIGN * z.b.rho;
+          one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.cs, t0, t1);
+          one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.sn, t1, t2);
+          one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.cs, t2, t3);
+          one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.sn, t3, t4);
+        } while (++b_lo != seg_end);
+        left -= seg;
+        if (seg == to_snap) {  // a frame is due after this block
+          store_snapshot(a.snap, a.snap_stride, k, s);
+          to_snap = K >> 2;
+        } else {
+          to_snap -= seg;
         }
-        const Real ra = Noise4<Real>::SIGN * z.a.rho, rb = Noise4<Real>::SIGN * z.b.rho;
-        one_step<Real, INTEG, TILT>(s, cf, ra, z.a.cs, t0, t1);
-        one_step<Real, INTEG, TILT>(s, cf, ra, z.a.sn, t1, t2);
-        one_step<Real, INTEG, TILT>(s, cf, rb, z.b.cs, t2, t3);
-        one_step<Real, INTEG, TILT>(s, cf, rb, z.b.sn, t3, t4);
-      } while (++b_lo != b_end);
+      } while (left);
       n += static_cast<uint64_t>(nb) << 2;
+      if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
     } else {
       // ---- slow path: one step (unaligned head / tail, or K not a multiple of 4) ----
       const uint4 w = philox_block(a.seed, id.global, n >> 2);
@@ -221,7 +248,7 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
         t0 = a.tilt[n - a.tilt_base];
         if (INTEG == 1) t1 = a.tilt[n - a.tilt_base + 1];
       }
-      one_step<Real, INTEG, TILT>(s, cf, rho, cs, t0, t1);
+      one_step<Real, INTEG, TILT, PRECISE>(s, cf, rho, cs, t0, t1);
       ++n;
     }
     if (n == next_snap) {
@@ -232,6 +259,7 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
   a.x[k] = s.x;
   a.v[k] = s.v;
   a.e[k] = s.e;
+  if (PRECISE) a.xl[k] = s.xl;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -296,10 +324,18 @@ __host__ __device__ inline void finalize_moment(const double* s, uint64_t step, 
   m->n = static_cast<uint64_t>(N);
   m->step = step;
   const double mx = s[1] / N, mv = s[3] / N;
+  // no FMA contraction: the device record and abm_moments_from_sums (host) agree bit for bit
+#ifdef __CUDA_ARCH__
+  const double mx2 = __dmul_rn(mx, mx), mv2 = __dmul_rn(mv, mv);
+  m->var_x = __dsub_rn(s[2] / N, mx2);
+  m->var_v = __dsub_rn(s[4] / N, mv2);
+#else
+  volatile double mx2 = mx * mx, mv2 = mv * mv;
+  m->var_x = s[2] / N - mx2;
+  m->var_v = s[4] / N - mv2;
+#endif
   m->mean_x = mx;
-  m->var_x = s[2] / N - mx * mx;
   m->mean_v = mv;
-  m->var_v = s[4] / N - mv * mv;
   m->mean_e = s[5] / N;
   m->mean_dx = s[6] / N;
   m->mean_dx2 = s[7] / N;

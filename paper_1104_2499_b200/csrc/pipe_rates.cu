@@ -31,26 +31,28 @@ constexpr int UNROLL = 8;   // CHAINS * UNROLL instructions (per class) per loop
 enum Op {
   FFMA_RRR, FFMA_RRC, FFMA_RIR, FMUL_RR, FADD_RR, IMAD_LO, IMAD_WIDE_R, IMAD_WIDE_I, LOP3_XOR3,
   IADD3, SHF_R, MUFU_COS, MUFU_SIN, MUFU_LG2, MUFU_SQRT, MUFU_RSQ, MUFU_EX2, MUFU_RCP,
-  DFMA_, DMUL_, DADD_, I2F_, F2I_, N_OPS
+  DFMA_, DMUL_, DADD_, I2F_, F2I_, FFMA2_, FRND_, N_OPS
 };
 static const char* OP_NAME[N_OPS] = {
   "FFMA r,r,r", "FFMA r,r,c[]", "FFMA r,imm,r", "FMUL r,r", "FADD r,r", "IMAD.LO r,r,r",
   "IMAD.WIDE.U32 r,r", "IMAD.WIDE r,imm + LOP3", "LOP3 (xor3)", "IADD3 r,r,r", "SHF.R",
   "FMUL+MUFU.COS", "FMUL+MUFU.SIN", "MUFU.LG2", "MUFU.SQRT", "MUFU.RSQ", "MUFU.EX2", "MUFU.RCP",
-  "DFMA", "DMUL", "DADD", "I2F.U32", "F2I.U32"};
+  "DFMA", "DMUL", "DADD", "I2F.U32", "F2I.U32", "FFMA2 (f32x2, per elem)", "FRND"};
 
 struct Regs {
   float f[CHAINS];
   uint32_t u[CHAINS];
   uint32_t h[CHAINS];
   double d[CHAINS];
+  unsigned long long p[CHAINS];
 };
 
 __constant__ float c_k[4];
 
 template <int OP>
 __device__ __forceinline__ void one(Regs& r, int j, float fb, float fc, uint32_t ub, uint32_t uc,
-                                    double db, double dc) {
+                                    double db, double dc, unsigned long long pb = 0,
+                                    unsigned long long pc = 0) {
   if (OP == FFMA_RRR) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(r.f[j]) : "f"(fb), "f"(fc));
   if (OP == FFMA_RRC) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(r.f[j]) : "f"(fb), "f"(c_k[1]));
   if (OP == FFMA_RIR) asm volatile("fma.rn.f32 %0, %0, 0f3F7FFFF0, %1;" : "+f"(r.f[j]) : "f"(fc));
@@ -81,14 +83,20 @@ __device__ __forceinline__ void one(Regs& r, int j, float fb, float fc, uint32_t
   if (OP == DMUL_) asm volatile("mul.rn.f64 %0, %0, %1;" : "+d"(r.d[j]) : "d"(db));
   if (OP == DADD_) asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(r.d[j]) : "d"(dc));
   if (OP == I2F_) asm volatile("{\n\t.reg .f32 t;\n\tcvt.rn.f32.u32 t, %0;\n\tmov.b32 %0, t;\n\t}" : "+r"(r.u[j]));
+  // packed pair of fp32 FMAs (sm_100 FFMA2): counted as TWO lane-ops per thread below
+  if (OP == FFMA2_) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(r.p[j]) : "l"(pb), "l"(pc));
+  if (OP == FRND_) asm volatile("cvt.rni.f32.f32 %0, %0;" : "+f"(r.f[j]));
   if (OP == F2I_) asm volatile("{\n\t.reg .u32 t;\n\tcvt.rzi.u32.f32 t, %0;\n\tmov.b32 %0, t;\n\t}" : "+f"(r.f[j]));
 }
 
 __host__ __device__ constexpr bool uses_f(int op) {
-  return op <= FADD_RR || (op >= MUFU_COS && op <= MUFU_RCP) || op == F2I_;
+  return op <= FADD_RR || (op >= MUFU_COS && op <= MUFU_RCP) || op == F2I_ || op == FRND_;
 }
 __host__ __device__ constexpr bool uses_d(int op) { return op >= DFMA_ && op <= DADD_; }
-__host__ __device__ constexpr bool uses_u(int op) { return op < N_OPS && !uses_f(op) && !uses_d(op); }
+__host__ __device__ constexpr bool uses_p(int op) { return op == FFMA2_; }
+__host__ __device__ constexpr bool uses_u(int op) {
+  return op < N_OPS && !uses_f(op) && !uses_d(op) && !uses_p(op);
+}
 
 template <int OP>
 __device__ __forceinline__ void init_regs(Regs& r, const float* in, int o) {
@@ -97,6 +105,10 @@ __device__ __forceinline__ void init_regs(Regs& r, const float* in, int o) {
     if (uses_f(OP)) r.f[j] = in[4 + o] + j + threadIdx.x;
     if (uses_u(OP)) { r.u[j] = __float_as_uint(in[5 + o]) + 3 * j + threadIdx.x; r.h[j] = 0; }
     if (uses_d(OP)) r.d[j] = static_cast<double>(in[4 + o]) + j + threadIdx.x;
+    if (uses_p(OP)) {
+      const float2 t = make_float2(in[4 + o] + j + threadIdx.x, in[5 + o] + j);
+      r.p[j] = *reinterpret_cast<const unsigned long long*>(&t);
+    }
   }
 }
 template <int OP>
@@ -106,6 +118,7 @@ __device__ __forceinline__ void fold_regs(const Regs& r, float& acc, uint32_t& u
     if (uses_f(OP)) acc += r.f[j];
     if (uses_u(OP)) ua ^= r.u[j] ^ r.h[j];
     if (uses_d(OP)) da += r.d[j];
+    if (uses_p(OP)) ua ^= static_cast<uint32_t>(r.p[j]) ^ static_cast<uint32_t>(r.p[j] >> 32);
   }
 }
 
@@ -118,6 +131,9 @@ __global__ void __launch_bounds__(1024) rate_kernel(int iters, const float* __re
   const float fb = in[0], fc = in[1];
   const uint32_t ub = __float_as_uint(in[2]) | 1u, uc = __float_as_uint(in[3]);
   const double db = static_cast<double>(in[0]), dc = static_cast<double>(in[1]);
+  const float2 fb2 = make_float2(fb, fb), fc2 = make_float2(fc, fc);
+  const unsigned long long pb = *reinterpret_cast<const unsigned long long*>(&fb2);
+  const unsigned long long pc = *reinterpret_cast<const unsigned long long*>(&fc2);
   init_regs<OPA>(a, in, 0);
   init_regs<OPB>(b, in, 2);
   __syncthreads();
@@ -128,8 +144,8 @@ __global__ void __launch_bounds__(1024) rate_kernel(int iters, const float* __re
     for (int u = 0; u < UNROLL; ++u) {
 #pragma unroll
       for (int j = 0; j < CHAINS; ++j) {
-        one<OPA>(a, j, fb, fc, ub, uc, db, dc);
-        if (OPB != N_OPS) one<OPB == N_OPS ? 0 : OPB>(b, j, fb, fc, ub, uc, db, dc);
+        one<OPA>(a, j, fb, fc, ub, uc, db, dc, pb, pc);
+        if (OPB != N_OPS) one<OPB == N_OPS ? 0 : OPB>(b, j, fb, fc, ub, uc, db, dc, pb, pc);
       }
     }
   }
@@ -169,13 +185,16 @@ void single(const Dev& d) {
   const double r8 = run<OP, N_OPS>(d, 256, 1, 2000);    // 2 warps / scheduler
   const double r16 = run<OP, N_OPS>(d, 512, 1, 2000);   // 4 warps / scheduler
   const double r32 = run<OP, N_OPS>(d, 1024, 1, 1000);  // 8 warps / scheduler
-  std::printf("%-22s %8.1f %8.1f %8.1f\n", OP_NAME[OP], r8, r16, r32);
+  const double w = OP == FFMA2_ ? 2.0 : 1.0;  // two fp32 FMAs per FFMA2
+  std::printf("%-22s %8.1f %8.1f %8.1f\n", OP_NAME[OP], w * r8, w * r16, w * r32);
 }
 
 template <int OPA, int OPB>
 void mix(const Dev& d) {
   const double r = run<OPA, OPB>(d, 1024, 1, 1000);
-  std::printf("%-22s + %-22s %8.1f each, %8.1f total\n", OP_NAME[OPA], OP_NAME[OPB], r, 2 * r);
+  const double wa = OPA == FFMA2_ ? 2.0 : 1.0, wb = OPB == FFMA2_ ? 2.0 : 1.0;
+  std::printf("%-24s + %-24s %8.1f / %8.1f, %8.1f total\n", OP_NAME[OPA], OP_NAME[OPB], wa * r, wb * r,
+              (wa + wb) * r);
 }
 
 int main() {
@@ -200,6 +219,7 @@ int main() {
   single<MUFU_COS>(d); single<MUFU_SIN>(d); single<MUFU_LG2>(d); single<MUFU_SQRT>(d);
   single<MUFU_RSQ>(d); single<MUFU_EX2>(d); single<MUFU_RCP>(d);
   single<DFMA_>(d); single<DMUL_>(d); single<DADD_>(d); single<I2F_>(d); single<F2I_>(d);
+  single<FFMA2_>(d); single<FRND_>(d);
   std::printf("# mixes, 32 warps/SM, one to one\n");
   mix<FFMA_RRR, LOP3_XOR3>(d);
   mix<FFMA_RRR, IMAD_WIDE_I>(d);
@@ -213,5 +233,15 @@ int main() {
   mix<DFMA_, FFMA_RRR>(d);
   mix<DFMA_, LOP3_XOR3>(d);
   mix<DFMA_, IMAD_WIDE_I>(d);
+  mix<FFMA2_, IMAD_WIDE_I>(d);
+  mix<FFMA2_, IMAD_LO>(d);
+  mix<FFMA2_, LOP3_XOR3>(d);
+  mix<FFMA2_, MUFU_COS>(d);
+  mix<FFMA2_, FFMA_RRR>(d);
+  mix<FRND_, FFMA_RRR>(d);
+  mix<FRND_, MUFU_LG2>(d);
+  mix<I2F_, MUFU_LG2>(d);
+  mix<I2F_, LOP3_XOR3>(d);
+  mix<I2F_, FFMA_RRR>(d);
   return 0;
 }
