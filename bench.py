@@ -53,7 +53,7 @@ def load_peaks():
 # clocks sampled DURING the timed region
 # ---------------------------------------------------------------------------------------------
 class ClockSampler:
-    def __init__(self, index=0, period=0.05):
+    def __init__(self, index=0, period=0.2):
         self.index, self.period = index, period
         self.sm, self.reasons, self.max_mhz = [], set(), None
         self._stop = threading.Event()

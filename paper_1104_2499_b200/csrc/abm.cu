@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -46,6 +47,7 @@ struct abm_ctx {
   double* partial;      // [n_sets * blocks_per_set][7]
   double* sums;         // [n_sets][8]
   MomentRec* moments;   // [n_sets]
+  void* host_coefs;     // host copy of the coefficient table (source of the async upload)
   void* frame;          // staging frame for abm_snapshot_host (lazily allocated)
   size_t frame_bytes;
   uint32_t mom_block, mom_slice, blocks_per_set;
@@ -147,27 +149,67 @@ int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets) {
   return ABM_OK;
 }
 
+// Device memory comes from a stream-ordered pool owned by the library (one per device, kept for
+// the life of the process, never trimmed): after the first context of a given size, abm_create /
+// abm_destroy cost microseconds and do not serialise against other users of the driver.
+constexpr int MAX_DEVICES = 64;
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pools[MAX_DEVICES] = {};
+
+cudaError_t pool_for(int device, cudaMemPool_t* out) {
+  if (device < 0 || device >= MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_pool_mutex);
+  if (!g_pools[device]) {
+    cudaMemPoolProps props;
+    std::memset(&props, 0, sizeof(props));
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = device;
+    cudaMemPool_t pool = nullptr;
+    cudaError_t e = cudaMemPoolCreate(&pool, &props);
+    if (e != cudaSuccess) return e;
+    uint64_t keep = ~0ull;
+    e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    if (e != cudaSuccess) {
+      cudaMemPoolDestroy(pool);
+      return e;
+    }
+    g_pools[device] = pool;
+  }
+  *out = g_pools[device];
+  return cudaSuccess;
+}
+
+cudaError_t dev_alloc(abm_ctx* c, void** p, size_t bytes) {
+  cudaMemPool_t pool = nullptr;
+  cudaError_t e = pool_for(c->device, &pool);
+  if (e != cudaSuccess) return e;
+  return cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, c->stream);
+}
+
+void dev_free(abm_ctx* c, void* p) {
+  if (p) cudaFreeAsync(p, c->stream);
+}
+
 void free_all(abm_ctx* c) {
-  cudaFree(c->x);
-  cudaFree(c->v);
-  cudaFree(c->e);
-  cudaFree(c->xl);
-  cudaFree(c->coef_table);
-  cudaFree(c->tilt_table);
-  cudaFree(c->partial);
-  cudaFree(c->sums);
-  cudaFree(c->moments);
-  cudaFree(c->frame);
+  void* all[] = {c->x, c->v, c->e, c->xl, c->coef_table, c->tilt_table, c->partial, c->sums,
+                 c->moments, c->frame};
+  for (void* p : all) dev_free(c, p);
+  std::free(c->host_coefs);
+  c->host_coefs = nullptr;
 }
 
 template <typename Real>
 int upload_coefs_and_init(abm_ctx* c, const abm_params* params) {
-  std::vector<Coef<Real>> tab(c->n_sets);
+  // the host copy lives as long as the context: the upload is asynchronous
+  Coef<Real>* tab = static_cast<Coef<Real>*>(std::malloc(sizeof(Coef<Real>) * c->n_sets));
+  if (!tab) return ABM_ENOMEM;
+  c->host_coefs = tab;
   for (uint32_t s = 0; s < c->n_sets; ++s) tab[s] = make_coef<Real>(params[s]);
-  ABM_CK(c, cudaMalloc(&c->coef_table, sizeof(Coef<Real>) * c->n_sets));
-  // synchronous copy from pageable memory: `tab` dies at return
-  ABM_CK(c, cudaMemcpy(c->coef_table, tab.data(), sizeof(Coef<Real>) * c->n_sets,
-                       cudaMemcpyHostToDevice));
+  ABM_CK(c, dev_alloc(c, &c->coef_table, sizeof(Coef<Real>) * c->n_sets));
+  ABM_CK(c, cudaMemcpyAsync(c->coef_table, tab, sizeof(Coef<Real>) * c->n_sets,
+                            cudaMemcpyHostToDevice, c->stream));
   const uint32_t grid = static_cast<uint32_t>((c->n_traj + 255) / 256);
   init_kernel<Real><<<grid, 256, 0, c->stream>>>(
       static_cast<Real*>(c->x), static_cast<Real*>(c->v), static_cast<Real*>(c->e),
@@ -227,6 +269,10 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
   a.snap_every = c->snap_every;
   a.snap_stride = c->snap_stride;
   a.coef0 = coef0<Real>(c);
+  const uint64_t g_first = c->traj_base;
+  const uint64_t g_last = c->traj_base + (c->n_sets - 1) * c->set_stride + (c->n_particles - 1);
+  a.traj_hi = static_cast<uint32_t>(g_first >> 32);
+  a.traj_hi_shared = (g_first >> 32) == (g_last >> 32) ? 1u : 0u;
   const uint32_t chunk_max = c->tilt ? TILT_CHUNK : MAX_LAUNCH_STEPS;
   while (n_steps > 0) {
     const uint32_t chunk = static_cast<uint32_t>(n_steps < chunk_max ? n_steps : chunk_max);
@@ -255,7 +301,7 @@ int reduce_moments(abm_ctx* c) {
       c->n_particles, c->traj_base, c->set_stride, c->seed, c->blocks_per_set, c->mom_slice,
       c->partial);
   ABM_CK(c, cudaGetLastError());
-  moments_final_kernel<<<(c->n_sets + 127) / 128, 128, 0, c->stream>>>(
+  moments_final_kernel<<<(c->n_sets + 3) / 4, 128, 0, c->stream>>>(  // one warp per set
       c->partial, c->n_sets, c->blocks_per_set, c->n_particles, c->step, c->sums, c->moments);
   ABM_CK(c, cudaGetLastError());
   return ABM_OK;
@@ -350,7 +396,7 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
     return code;
   };
   auto alloc = [&](void** p, size_t bytes) {
-    cudaError_t e = cudaMalloc(p, bytes);
+    cudaError_t e = dev_alloc(c, p, bytes);
     if (e != cudaSuccess) {
       rc = e == cudaErrorMemoryAllocation ? ABM_ENOMEM : ABM_ECUDA;
       cudaGetLastError();
@@ -406,11 +452,10 @@ int abm_snapshot_host(abm_ctx* c, void* host_ptr, size_t stride_bytes) {
   if (!host_ptr || !stride_ok(c, stride_bytes)) return ABM_EINVAL;
   const size_t bytes = stride_bytes * c->n_traj;
   if (c->frame_bytes < bytes) {
-    ABM_CK(c, cudaStreamSynchronize(c->stream));
-    cudaFree(c->frame);
+    dev_free(c, c->frame);
     c->frame = nullptr;
     c->frame_bytes = 0;
-    ABM_CK(c, cudaMalloc(&c->frame, bytes));
+    ABM_CK(c, dev_alloc(c, &c->frame, bytes));
     c->frame_bytes = bytes;
   }
   const int rc = write_frame(c, c->frame, static_cast<uint32_t>(stride_bytes));

@@ -5,8 +5,14 @@
 
 namespace abm {
 
-constexpr int STEP_BLOCK = 128;   // threads per CTA of the step kernel
-constexpr int STEP_MIN_BLOCKS = 12;  // resident CTAs per SM the register budget allows (40 regs)
+#ifndef ABM_STEP_BLOCK
+#define ABM_STEP_BLOCK 128
+#endif
+#ifndef ABM_STEP_MIN_BLOCKS
+#define ABM_STEP_MIN_BLOCKS 12
+#endif
+constexpr int STEP_BLOCK = ABM_STEP_BLOCK;   // threads per CTA of the step kernel
+constexpr int STEP_MIN_BLOCKS = ABM_STEP_MIN_BLOCKS;  // resident CTAs per SM (12 x 128 threads: 40 regs)
 constexpr int MOM_BLOCK = 256;    // threads per CTA of the moment reduction (max)
 constexpr int MOM_PER_THREAD = 16;
 constexpr int N_SUMS = 8;
@@ -29,6 +35,8 @@ struct StepArgs {
   uint32_t n_steps;              // steps in this launch
   uint32_t snap_every;           // K (0 = never)
   uint32_t snap_stride;          // bytes per trajectory in snap
+  uint32_t traj_hi;              // high word of every global trajectory index, if shared
+  uint32_t traj_hi_shared;       // 1: all trajectories of the launch share traj_hi
   Coef<Real> coef0;              // the single set's coefficients (used when UNIFORM)
 };
 
@@ -150,27 +158,16 @@ __device__ __forceinline__ void one_step(State<Real>& s, const Coef<Real>& k, Re
   }
 }
 
-template <typename Real, int INTEG, bool TILT, bool UNIFORM, bool PRECISE>
-__global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const __grid_constant__ StepArgs<Real> a) {
-  const uint64_t k = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
-  if (k >= a.n_traj) return;
-  const TrajId id = traj_id(k, a.n_particles, a.traj_base, a.set_stride, UNIFORM);
-  Coef<Real> cf = UNIFORM ? a.coef0 : a.coef_table[id.set];
-  if (UNIFORM) {
-    // Kernel-parameter coefficients are uniform operands and an FMA takes at most one of those.
-    // One operand of each uniform pair -- (d, c), (d, gamma0), (k2, k1), (th_s, th_o) -- and the
-    // Box-Muller angle offset are therefore read from the table in global memory instead: a
-    // loaded value stays in a register for the whole loop, whereas ptxas re-materialises
-    // constant-bank values with an LDC / MOV per use.
-    const Coef<Real>* g = a.coef_table;
-    cf.d = g->d;
-    cf.k1 = g->k1;
-    cf.th_o = g->th_o;
-    cf.bm_o = g->bm_o;
-  }
-
-  State<Real> s{a.x[k], a.v[k], a.e[k], PRECISE ? a.xl[k] : Real(0)};
-
+// The step loop of one trajectory.  traj_hi (the high word of the global trajectory index, Philox
+// counter word 3) is a separate argument so that the kernel can pass a kernel parameter when the
+// whole launch shares it: ptxas then knows that counter words 0, 1 and 3 and
+// the key are warp-uniform, keeps the first-round product M0 * b and the second-round product
+// M1 * c2' in the uniform datapath, and hoists the per-thread products M1 * traj_lo and M0 * c0'
+// out of the block loop: 16 instead of 20 IMAD.WIDE per Philox block on the vector pipes.
+template <typename Real, int INTEG, bool TILT, bool PRECISE>
+__device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_t k,
+                                          const uint32_t traj_lo, const uint32_t traj_hi,
+                                          const Coef<Real>& cf, State<Real>& s) {
   uint64_t n = a.step0;
   const uint64_t n_end = a.step0 + a.n_steps;
   const uint32_t K = a.snap != nullptr ? a.snap_every : 0u;
@@ -200,16 +197,16 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
       // IMAD.WIDE / LOP3 (fmaheavy + alu pipes) and FFMA / MUFU (fma + xu pipes) instead of an
       // integer phase followed by a floating-point phase.  The block after the last one of this
       // run is computed and dropped (its counter may wrap: harmless).
-      uint4 w = philox4x32_10(b_lo, b_hi, static_cast<uint32_t>(id.global),
-                              static_cast<uint32_t>(id.global >> 32),
+      uint4 w = philox4x32_10(b_lo, b_hi, traj_lo,
+                              traj_hi,
                               static_cast<uint32_t>(a.seed), static_cast<uint32_t>(a.seed >> 32));
       do {
         const uint32_t seg = left < to_snap ? left : static_cast<uint32_t>(to_snap);  // >= 1
         const uint32_t seg_end = b_lo + seg;  // may wrap to 0: the loop runs until equality
 #pragma unroll 1
         do {
-          const uint4 w_next = philox4x32_10(b_lo + 1u, b_hi, static_cast<uint32_t>(id.global),
-                                             static_cast<uint32_t>(id.global >> 32),
+          const uint4 w_next = philox4x32_10(b_lo + 1u, b_hi, traj_lo,
+                                             traj_hi,
                                              static_cast<uint32_t>(a.seed),
                                              static_cast<uint32_t>(a.seed >> 32));
           const Noise4<Real> z(w, cf);
@@ -238,7 +235,7 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
       if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
     } else {
       // ---- slow path: one step (unaligned head / tail, or K not a multiple of 4) ----
-      const uint4 w = philox_block(a.seed, id.global, n >> 2);
+      const uint4 w = philox_block(a.seed, (static_cast<uint64_t>(traj_hi) << 32) | traj_lo, n >> 2);
       const Noise4<Real> z(w, cf);
       const bool second = (n >> 1) & 1u;
       const Real rho = Noise4<Real>::SIGN * (second ? z.b.rho : z.a.rho);
@@ -256,6 +253,38 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
       next_snap += K;
     }
   }
+}
+
+template <typename Real, int INTEG, bool TILT, bool UNIFORM, bool PRECISE>
+__global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const __grid_constant__ StepArgs<Real> a) {
+  const uint64_t k = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
+  if (k >= a.n_traj) return;
+  const TrajId id = traj_id(k, a.n_particles, a.traj_base, a.set_stride, UNIFORM);
+  Coef<Real> cf = UNIFORM ? a.coef0 : a.coef_table[id.set];
+  if (UNIFORM) {
+    // Kernel-parameter coefficients are uniform operands and an FMA takes at most one of those.
+    // One operand of each uniform pair -- (d, c), (d, gamma0), (k2, k1), (th_s, th_o) -- and the
+    // Box-Muller angle offset are therefore read from the table in global memory instead: a
+    // loaded value stays in a register for the whole loop, whereas ptxas re-materialises
+    // constant-bank values with an LDC / MOV per use.
+    const Coef<Real>* g = a.coef_table;
+    cf.d = g->d;
+    cf.k1 = g->k1;
+    cf.th_o = g->th_o;
+    cf.bm_o = g->bm_o;
+  }
+
+  State<Real> s{a.x[k], a.v[k], a.e[k], PRECISE ? a.xl[k] : Real(0)};
+
+  // High word of the global trajectory index (Philox counter word 3): the host passes it as a
+  // kernel parameter when the whole launch shares one value (always, unless the index range
+  // straddles a multiple of 2^32), which makes it a uniform-register operand.
+  if (a.traj_hi_shared)
+    run_steps<Real, INTEG, TILT, PRECISE>(a, k, static_cast<uint32_t>(id.global), a.traj_hi, cf, s);
+  else
+    run_steps<Real, INTEG, TILT, PRECISE>(a, k, static_cast<uint32_t>(id.global),
+                                          static_cast<uint32_t>(id.global >> 32), cf, s);
+
   a.x[k] = s.x;
   a.v[k] = s.v;
   a.e[k] = s.e;
@@ -342,19 +371,31 @@ __host__ __device__ inline void finalize_moment(const double* s, uint64_t step, 
   m->mean_x2 = s[2] / N;
 }
 
-__global__ void moments_final_kernel(const double* __restrict__ partial, uint32_t n_sets,
-                                     uint32_t blocks_per_set, uint64_t n_particles, uint64_t step,
-                                     double* __restrict__ sums, MomentRec* __restrict__ out) {
-  const uint32_t set = blockIdx.x * blockDim.x + threadIdx.x;
-  if (set >= n_sets) return;
+// One warp per set: lane l adds the CTA partials l, l + 32, ... in index order, then a fixed
+// xor-shuffle tree; lane 0 finalises.
+__global__ void __launch_bounds__(128)
+moments_final_kernel(const double* __restrict__ partial, uint32_t n_sets, uint32_t blocks_per_set,
+                     uint64_t n_particles, uint64_t step, double* __restrict__ sums,
+                     MomentRec* __restrict__ out) {
+  const uint32_t set = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const uint32_t lane = threadIdx.x & 31u;
+  if (set >= n_sets) return;  // whole warps leave together
   double s[N_SUMS];
   s[0] = static_cast<double>(n_particles);
-  for (int q = 1; q < N_SUMS; ++q) s[q] = 0;
   const double* p = partial + static_cast<uint64_t>(set) * blocks_per_set * (N_SUMS - 1);
-  for (uint32_t b = 0; b < blocks_per_set; ++b)
-    for (int q = 0; q < N_SUMS - 1; ++q) s[q + 1] += p[static_cast<uint64_t>(b) * (N_SUMS - 1) + q];
-  for (int q = 0; q < N_SUMS; ++q) sums[static_cast<uint64_t>(set) * N_SUMS + q] = s[q];
-  finalize_moment(s, step, &out[set]);
+#pragma unroll
+  for (int q = 0; q < N_SUMS - 1; ++q) {
+    double t = 0;
+    for (uint32_t b = lane; b < blocks_per_set; b += 32)
+      t += p[static_cast<uint64_t>(b) * (N_SUMS - 1) + q];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) t += __shfl_xor_sync(0xffffffffu, t, off);
+    s[q + 1] = t;
+  }
+  if (lane == 0) {
+    for (int q = 0; q < N_SUMS; ++q) sums[static_cast<uint64_t>(set) * N_SUMS + q] = s[q];
+    finalize_moment(s, step, &out[set]);
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
