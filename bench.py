@@ -178,7 +178,7 @@ def run_reference(args, wl):
 def run_ours(args, wl, cfg_id):
     import torch
     import torch.distributed as dist
-    from paper_1104_2499_b200 import binding as abm
+    from paper_1104_2499_b200 import binding as abm, sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -194,8 +194,9 @@ def run_ours(args, wl, cfg_id):
     stream = torch.cuda.Stream()
     sets = [wl.set_params(s) for s in range(wl.n_param_sets)]
     T = wl.n_trajectories
-    # weak scaling: rank r owns global trajectories [r*T, (r+1)*T); whole sets stay on one rank
-    traj_base = rank * T
+    # weak scaling: rank r integrates a full copy of the workload on global trajectories [r*T, (r+1)*T)
+    plan = sharding.shard_plan(wl.n_particles, wl.n_param_sets, rank, world, "weak")
+    traj_base = plan.traj_base
     n_steps, M = wl.n_steps, (wl.moments_every or wl.n_steps)
     fp64 = sets[0]["precision"] == 1
     frame_cols = 2
@@ -227,10 +228,8 @@ def run_ours(args, wl, cfg_id):
                 if ev is not None:
                     ev[1].record(stream)
                 launches["n"] += step_launches
-                if world > 1:
-                    sums = torch.from_numpy(ens.moment_sums()).cuda()          # S6 (2 kernels)
-                    dist.all_reduce(sums)
-                    m = abm.abm_moments_from_sums(sums.cpu().numpy(), ens.step_count)
+                if world > 1:                                                  # S6 (2 kernels) + NCCL
+                    m = sharding.reduce_moments(ens.moment_sums(), ens.step_count, plan, device="cuda")
                 else:
                     m = ens.moments()                                          # S6 (2 kernels)
                 launches["n"] += 2
