@@ -45,6 +45,65 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
   return make_uint4(c0, c1, c2, c3);
 }
 
+// One Philox round with round key (k0, k1).
+__device__ __forceinline__ void philox_round(uint32_t& c0, uint32_t& c1, uint32_t& c2, uint32_t& c3,
+                                             uint32_t k0, uint32_t k1) {
+  uint32_t hi0, lo0, hi1, lo1;
+  mul_wide(c0, PHILOX_M0, hi0, lo0);
+  mul_wide(c2, PHILOX_M1, hi1, lo1);
+  c0 = hi1 ^ c1 ^ k0;
+  c1 = lo1;
+  c2 = hi0 ^ c3 ^ k1;
+  c3 = lo0;
+}
+
+// The first two rounds split by what their inputs depend on, for a run of blocks b = (b_lo, b_hi)
+// of ONE trajectory with b_hi fixed ("Philox block table"):
+//   after round 0:  c0' = hi(M1 t_lo) ^ b_hi ^ k0      per trajectory, the same for every block
+//                   c1' = lo(M1 t_lo)                  per trajectory
+//                   c2' = hi(M0 b_lo) ^ t_hi ^ k1      per block, the same for every trajectory
+//                   c3' = lo(M0 b_lo)                  per block
+//   after round 1:  c0'' = [hi(M1 c2') ^ k0_1] ^ c1'   c1'' = lo(M1 c2')
+//                   c2'' = hi(M0 c0') ^ [c3' ^ k1_1]   c3'' = lo(M0 c0')
+// PhiloxTraj holds the per-trajectory words (2 multiplies, once per run); PhiloxBlockHead holds
+// the bracketed per-block words (2 multiplies per block, shared by all trajectories whose t_hi is
+// equal -- the step kernel keeps them in a shared-memory table computed once per CTA).
+struct PhiloxTraj {
+  uint32_t p1, p2, p3;  // c1', hi(M0 c0'), lo(M0 c0')
+};
+struct PhiloxBlockHead {
+  uint32_t u0, u1, u2;  // hi(M1 c2') ^ k0_1, lo(M1 c2'), c3' ^ k1_1
+};
+__device__ __forceinline__ PhiloxTraj philox_traj(uint32_t t_lo, uint32_t b_hi, uint32_t k0) {
+  uint32_t h1, l1;
+  mul_wide(t_lo, PHILOX_M1, h1, l1);
+  PhiloxTraj t;
+  t.p1 = l1;
+  mul_wide(h1 ^ b_hi ^ k0, PHILOX_M0, t.p2, t.p3);
+  return t;
+}
+__device__ __forceinline__ PhiloxBlockHead philox_block_head(uint32_t b_lo, uint32_t t_hi,
+                                                             uint32_t k0, uint32_t k1) {
+  uint32_t h0, l0, h1, l1;
+  mul_wide(b_lo, PHILOX_M0, h0, l0);
+  mul_wide(h0 ^ t_hi ^ k1, PHILOX_M1, h1, l1);
+  PhiloxBlockHead u;
+  u.u0 = h1 ^ (k0 + PHILOX_W0);
+  u.u1 = l1;
+  u.u2 = l0 ^ (k1 + PHILOX_W1);
+  return u;
+}
+// Rounds 2..9 on the state after round 1 assembled from the two halves.
+__device__ __forceinline__ uint4 philox_finish(const PhiloxTraj& t, uint32_t u0, uint32_t u1,
+                                               uint32_t u2, uint32_t k0, uint32_t k1) {
+  uint32_t c0 = u0 ^ t.p1, c1 = u1, c2 = t.p2 ^ u2, c3 = t.p3;
+#pragma unroll
+  for (int r = 2; r < 10; ++r)
+    philox_round(c0, c1, c2, c3, k0 + PHILOX_W0 * static_cast<uint32_t>(r),
+                 k1 + PHILOX_W1 * static_cast<uint32_t>(r));
+  return make_uint4(c0, c1, c2, c3);
+}
+
 // Stream layout: key = (seed lo, seed hi),
 // ctr = (block lo, block hi, trajectory lo, trajectory hi).
 __device__ __forceinline__ uint4 philox_block(uint64_t seed, uint64_t traj, uint64_t b) {

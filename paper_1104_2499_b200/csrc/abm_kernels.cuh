@@ -8,11 +8,32 @@ namespace abm {
 #ifndef ABM_STEP_BLOCK
 #define ABM_STEP_BLOCK 128
 #endif
-#ifndef ABM_STEP_MIN_BLOCKS
-#define ABM_STEP_MIN_BLOCKS 12
+// Resident CTAs per SM of the step kernel (the register cap follows: 65,536 / (128 * n)), per
+// kernel family.  The loop is bound by the FMA dispatch port, not by latency, so 6-8 warps per
+// scheduler are enough; what matters is (i) no spills in the loop and (ii) little wave
+// quantisation: all CTAs run equally long, so T / (148 * 128 * n) waves round UP
+// (config[1]: n = 12 -> 4.61 waves cost 5; n = 8 -> 6.92 cost 7).
+// Measured on B200 (steady state, round-1 sweeps): fp32 EM one set 8 > 7 > 6 > 12;
+// fp32 Heun 5 ~ 4 > 6 > 8; fp32 with per-thread coefficients 4 > 6 > 8 > 12 (12 spilled 236 B);
+// fp64 insensitive between 4 and 8 (12 spilled > 1 KB).
+#ifndef ABM_MINB_F32U
+#define ABM_MINB_F32U 8   // fp32 Euler-Maruyama, one parameter set (uniform coefficients): <= 64 regs
+#endif
+#ifndef ABM_MINB_F32H
+#define ABM_MINB_F32H 5   // fp32 Heun, one parameter set: <= 96 regs
+#endif
+#ifndef ABM_MINB_F32N
+#define ABM_MINB_F32N 4   // fp32, per-thread coefficient record (config[2]): <= 128 regs
+#endif
+#ifndef ABM_MINB_F64
+#define ABM_MINB_F64 8    // fp64: <= 64 regs
 #endif
 constexpr int STEP_BLOCK = ABM_STEP_BLOCK;   // threads per CTA of the step kernel
-constexpr int STEP_MIN_BLOCKS = ABM_STEP_MIN_BLOCKS;  // resident CTAs per SM (12 x 128 threads: 40 regs)
+template <typename Real, int INTEG, bool UNIFORM>
+constexpr int step_min_blocks() {
+  return sizeof(Real) == 8 ? ABM_MINB_F64
+                           : (!UNIFORM ? ABM_MINB_F32N : (INTEG == 1 ? ABM_MINB_F32H : ABM_MINB_F32U));
+}
 constexpr int MOM_BLOCK = 256;    // threads per CTA of the moment reduction (max)
 constexpr int MOM_PER_THREAD = 16;
 constexpr int N_SUMS = 8;
@@ -158,16 +179,50 @@ __device__ __forceinline__ void one_step(State<Real>& s, const Coef<Real>& k, Re
   }
 }
 
-// The step loop of one trajectory.  traj_hi (the high word of the global trajectory index, Philox
-// counter word 3) is a separate argument so that the kernel can pass a kernel parameter when the
-// whole launch shares it: ptxas then knows that counter words 0, 1 and 3 and
-// the key are warp-uniform, keeps the first-round product M0 * b and the second-round product
-// M1 * c2' in the uniform datapath, and hoists the per-thread products M1 * traj_lo and M0 * c0'
-// out of the block loop: 16 instead of 20 IMAD.WIDE per Philox block on the vector pipes.
+// Four steps from one Philox block.
 template <typename Real, int INTEG, bool TILT, bool PRECISE>
-__device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_t k,
+__device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf, const uint4& w,
+                                           const Real*& tl) {
+  const Noise4<Real> z(w, cf);
+  Real t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0;
+  if (TILT) {
+    t0 = tl[0]; t1 = tl[1]; t2 = tl[2]; t3 = tl[3];
+    if (INTEG == 1) t4 = tl[4];
+    tl += 4;
+  }
+  const Real ra = Noise4<Real>::SIGN * z.a.rho, rb = Noise4<Real>::SIGN * z.b.rho;
+  one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.cs, t0, t1);
+  one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.sn, t1, t2);
+  one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.cs, t2, t3);
+  one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.sn, t3, t4);
+}
+
+// The step loop of one trajectory.
+//
+// TABLE (the whole launch shares traj_hi, the high word of the global trajectory index = Philox
+// counter word 3): the half of the first two Philox rounds that depends only on the block index --
+// two of the 20 multiplies -- is the same for every trajectory, so each CTA computes it once per
+// block into a shared-memory table (PHILOX_CHUNK blocks per refill, one entry per thread, double
+// buffered: one __syncthreads per refill) and every thread fetches its entry with one broadcast
+// LDS.128.  Two more multiplies depend only on the trajectory and are done once per run.  16
+// IMAD.WIDE per block remain per thread.  IMAD.WIDE runs at a quarter of the FFMA rate on the
+// FFMA dispatch port (profiles/r01_pipe_rates.txt), so multiplies are what this loop is short of.
+// All threads of a CTA execute the same loop (bounds are launch-uniform); threads past the end of
+// the ensemble integrate a copy of the last trajectory and store nothing (`active`).
+//
+// Software pipeline: the Philox block of the NEXT four steps is computed next to the
+// floating-point work of the current four, so every warp issues a steady mix of IMAD.WIDE / LOP3
+// and FFMA / MUFU instead of an integer phase followed by a floating-point phase.  The block
+// after the last one of a run is computed and dropped (its counter may wrap: harmless).
+constexpr int PHILOX_CHUNK = STEP_BLOCK;  // table entries per refill = threads per CTA
+
+template <typename Real, int INTEG, bool TILT, bool PRECISE, bool TABLE>
+__device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_t k, const bool active,
                                           const uint32_t traj_lo, const uint32_t traj_hi,
                                           const Coef<Real>& cf, State<Real>& s) {
+  __shared__ uint4 tab[TABLE ? 2 : 1][TABLE ? PHILOX_CHUNK : 1];
+  uint32_t par = 0;
+  const uint32_t k0 = static_cast<uint32_t>(a.seed), k1 = static_cast<uint32_t>(a.seed >> 32);
   uint64_t n = a.step0;
   const uint64_t n_end = a.step0 + a.n_steps;
   const uint32_t K = a.snap != nullptr ? a.snap_every : 0u;
@@ -175,7 +230,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
   if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
 
   // Frames fall on Philox-block boundaries when K is a multiple of 4 (n is a multiple of 4 on the
-  // fast path): they are then stored from inside the block loop and the software pipeline below
+  // fast path): they are then stored from inside the block loop and the software pipeline
   // runs through them.  Otherwise a run of whole blocks ends at the next frame.
   const bool snap_aligned = (K & 3u) == 0;
   while (n < n_end) {
@@ -192,45 +247,61 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
       const Real* tl = TILT ? a.tilt + (n - a.tilt_base) : nullptr;
       uint64_t to_snap = (K && snap_aligned) ? (next_snap - n) >> 2 : ~0ull;  // blocks to the frame
       uint32_t left = nb;
-      // Software pipeline: the Philox block of the NEXT four steps is computed next to the
-      // floating-point work of the current four, so every warp issues a steady mix of
-      // IMAD.WIDE / LOP3 (fmaheavy + alu pipes) and FFMA / MUFU (fma + xu pipes) instead of an
-      // integer phase followed by a floating-point phase.  The block after the last one of this
-      // run is computed and dropped (its counter may wrap: harmless).
-      uint4 w = philox4x32_10(b_lo, b_hi, traj_lo,
-                              traj_hi,
-                              static_cast<uint32_t>(a.seed), static_cast<uint32_t>(a.seed >> 32));
-      do {
-        const uint32_t seg = left < to_snap ? left : static_cast<uint32_t>(to_snap);  // >= 1
-        const uint32_t seg_end = b_lo + seg;  // may wrap to 0: the loop runs until equality
-#pragma unroll 1
+      uint4 w = philox4x32_10(b_lo, b_hi, traj_lo, traj_hi, k0, k1);
+      if (TABLE) {
+        const PhiloxTraj pt = philox_traj(traj_lo, b_hi, k0);
         do {
-          const uint4 w_next = philox4x32_10(b_lo + 1u, b_hi, traj_lo,
-                                             traj_hi,
-                                             static_cast<uint32_t>(a.seed),
-                                             static_cast<uint32_t>(a.seed >> 32));
-          const Noise4<Real> z(w, cf);
-          w = w_next;
-          Real t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0;
-          if (TILT) {
-            t0 = tl[0]; t1 = tl[1]; t2 = tl[2]; t3 = tl[3];
-            if (INTEG == 1) t4 = tl[4];
-            tl += 4;
+          // refill: entry j belongs to block b_lo + 1 + j (the block the pipeline computes in
+          // iteration j of this chunk)
+          const PhiloxBlockHead h = philox_block_head(b_lo + 1u + threadIdx.x, traj_hi, k0, k1);
+          tab[par][threadIdx.x] = make_uint4(h.u0, h.u1, h.u2, 0u);
+          __syncthreads();
+          const uint32_t in_chunk = left < static_cast<uint32_t>(PHILOX_CHUNK)
+                                        ? left : static_cast<uint32_t>(PHILOX_CHUNK);
+          const uint4* tp = tab[par];
+          uint32_t done = 0;
+          do {
+            const uint32_t rest = in_chunk - done;
+            const uint32_t seg = rest < to_snap ? rest : static_cast<uint32_t>(to_snap);  // >= 1
+            const uint4* const tp_end = tp + seg;
+#pragma unroll 1
+            do {
+              const uint4 u = *tp;
+              const uint4 w_next = philox_finish(pt, u.x, u.y, u.z, k0, k1);
+              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+              w = w_next;
+            } while (++tp != tp_end);
+            done += seg;
+            if (seg == to_snap) {  // a frame is due after this block
+              if (active) store_snapshot(a.snap, a.snap_stride, k, s);
+              to_snap = K >> 2;
+            } else {
+              to_snap -= seg;
+            }
+          } while (done != in_chunk);
+          left -= in_chunk;
+          b_lo += in_chunk;
+          par ^= 1u;
+        } while (left);
+      } else {
+        do {
+          const uint32_t seg = left < to_snap ? left : static_cast<uint32_t>(to_snap);  // >= 1
+          const uint32_t seg_end = b_lo + seg;  // may wrap to 0: the loop runs until equality
+#pragma unroll 1
+          do {
+            const uint4 w_next = philox4x32_10(b_lo + 1u, b_hi, traj_lo, traj_hi, k0, k1);
+            four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+            w = w_next;
+          } while (++b_lo != seg_end);
+          left -= seg;
+          if (seg == to_snap) {  // a frame is due after this block
+            if (active) store_snapshot(a.snap, a.snap_stride, k, s);
+            to_snap = K >> 2;
+          } else {
+            to_snap -= seg;
           }
-          const Real ra = Noise4<Real>::SIGN * z.a.rho, rb = Noise4<Real>::SIGN * z.b.rho;
-          one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.cs, t0, t1);
-          one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.sn, t1, t2);
-          one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.cs, t2, t3);
-          one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.sn, t3, t4);
-        } while (++b_lo != seg_end);
-        left -= seg;
-        if (seg == to_snap) {  // a frame is due after this block
-          store_snapshot(a.snap, a.snap_stride, k, s);
-          to_snap = K >> 2;
-        } else {
-          to_snap -= seg;
-        }
-      } while (left);
+        } while (left);
+      }
       n += static_cast<uint64_t>(nb) << 2;
       if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
     } else {
@@ -249,16 +320,22 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
       ++n;
     }
     if (n == next_snap) {
-      store_snapshot(a.snap, a.snap_stride, k, s);
+      if (active) store_snapshot(a.snap, a.snap_stride, k, s);
       next_snap += K;
     }
   }
 }
 
+#ifndef ABM_PHILOX_TABLE
+#define ABM_PHILOX_TABLE 1
+#endif
+
 template <typename Real, int INTEG, bool TILT, bool UNIFORM, bool PRECISE>
-__global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const __grid_constant__ StepArgs<Real> a) {
-  const uint64_t k = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
-  if (k >= a.n_traj) return;
+__global__ void __launch_bounds__(STEP_BLOCK, step_min_blocks<Real, INTEG, UNIFORM>())
+step_kernel(const __grid_constant__ StepArgs<Real> a) {
+  const uint64_t k_raw = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
+  const bool active = k_raw < a.n_traj;
+  const uint64_t k = active ? k_raw : a.n_traj - 1;  // idle threads shadow the last trajectory
   const TrajId id = traj_id(k, a.n_particles, a.traj_base, a.set_stride, UNIFORM);
   Coef<Real> cf = UNIFORM ? a.coef0 : a.coef_table[id.set];
   if (UNIFORM) {
@@ -278,17 +355,20 @@ __global__ void __launch_bounds__(STEP_BLOCK, STEP_MIN_BLOCKS) step_kernel(const
 
   // High word of the global trajectory index (Philox counter word 3): the host passes it as a
   // kernel parameter when the whole launch shares one value (always, unless the index range
-  // straddles a multiple of 2^32), which makes it a uniform-register operand.
+  // straddles a multiple of 2^32); the block-head table of run_steps needs that.
   if (a.traj_hi_shared)
-    run_steps<Real, INTEG, TILT, PRECISE>(a, k, static_cast<uint32_t>(id.global), a.traj_hi, cf, s);
+    run_steps<Real, INTEG, TILT, PRECISE, ABM_PHILOX_TABLE != 0>(
+        a, k, active, static_cast<uint32_t>(id.global), a.traj_hi, cf, s);
   else
-    run_steps<Real, INTEG, TILT, PRECISE>(a, k, static_cast<uint32_t>(id.global),
-                                          static_cast<uint32_t>(id.global >> 32), cf, s);
+    run_steps<Real, INTEG, TILT, PRECISE, false>(a, k, active, static_cast<uint32_t>(id.global),
+                                                 static_cast<uint32_t>(id.global >> 32), cf, s);
 
-  a.x[k] = s.x;
-  a.v[k] = s.v;
-  a.e[k] = s.e;
-  if (PRECISE) a.xl[k] = s.xl;
+  if (active) {
+    a.x[k] = s.x;
+    a.v[k] = s.v;
+    a.e[k] = s.e;
+    if (PRECISE) a.xl[k] = s.xl;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
