@@ -221,12 +221,12 @@ def run_ours(args, wl, cfg_id):
                 ens.bind_snapshot()                                            # S5 (1 kernel)
                 launches["n"] += 1
             m = None
-            for _ in range(n_steps // M):
+            for j in range(n_steps // M):
                 if ev is not None:
-                    ev[0].record(stream)
+                    ev[j][0].record(stream)
                 ens.step(M)                                                    # S1-S5, S7
                 if ev is not None:
-                    ev[1].record(stream)
+                    ev[j][1].record(stream)
                 launches["n"] += step_launches
                 if world > 1:                                                  # S6 (2 kernels) + NCCL
                     m = sharding.reduce_moments(ens.moment_sums(), ens.step_count, plan, device="cuda")
@@ -252,8 +252,8 @@ def run_ours(args, wl, cfg_id):
     # ---- device-timed arm -------------------------------------------------------------------
     ev_pass = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
                for _ in range(args.steps)]
-    ev_kern = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-               for _ in range(args.steps)]
+    ev_kern = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                for _ in range(n_steps // M)] for _ in range(args.steps)]   # around every abm_step
     launches["n"] = 0
     barrier()
     wall0 = time.perf_counter()
@@ -262,14 +262,14 @@ def run_ours(args, wl, cfg_id):
             flush.fill_(i & 0xff)                       # L2 flush between timed iterations
             torch.cuda.synchronize()
             ev_pass[i][0].record(stream)
-            m = one_pass(False, ev_kern[i] if n_steps == M else None)
+            m = one_pass(False, ev_kern[i])
             ev_pass[i][1].record(stream)
         barrier()
     wall = time.perf_counter() - wall0
     gpu_launches = launches["n"]
     t_pass_ms = [a.elapsed_time(b) for a, b in ev_pass]
     t_dev = sum(t_pass_ms) * 1e-3
-    t_kern_ms = [a.elapsed_time(b) for a, b in ev_kern] if n_steps == M else None
+    t_kern_ms = [sum(a.elapsed_time(b) for a, b in evs) for evs in ev_kern]   # per pass, all abm_step calls
 
     # ---- end-to-end arm (host params -> host frame + moments), wall clock ---------------------
     barrier()
@@ -323,8 +323,9 @@ def run_ours(args, wl, cfg_id):
             "frac": achieved / peak,
             "frac_at_sustained_clock": achieved / (N_SM * LANES_PER_SM * sm_mhz * 1e6),
             "i_alg_per_particle_step": I_ALG[cfg_id],
-            "particle_steps_per_launch": wl.particle_steps,
-            "kernel_ms": 1e3 * t_k, "kernel_share_of_pass": sum(t_kern_ms) / sum(t_pass_ms),
+            "particle_steps_per_pass": wl.particle_steps,
+            "kernel_ms": 1e3 * t_k, "kernel_launches_per_pass": step_launches * (n_steps // M),
+            "kernel_share_of_pass": sum(t_kern_ms) / sum(t_pass_ms),
             "peak_source": f"148 SMs x 128 lanes x sm_max_mhz {f_max / 1e6:.0f} MHz, {peak_src}",
             "traffic": None,
             "hbm_algorithmic_bytes_per_launch": int(T * (24 + 8 * (n_steps // wl.snapshot_every

@@ -145,6 +145,32 @@ int abm_moment_sums(abm_ctx* ctx, double* out);
 int abm_moments_from_sums(const double* sums, uint32_t n_param_sets, uint64_t step,
                           abm_moment* out_moments);
 
+/* The quantity the paper plots (Fig. 2: mean velocity against the load force, "over
+ * time, results ... are averaged", :74): the velocity of each set averaged over its realisations AND
+ * over the time since step 0 (hence over all launches so far),
+ *     out[s] = < x(t) - x(0) >_s / (step * dt)
+ * -- for Euler-Maruyama x(t) - x(0) = dt * (sum of v over the steps) exactly, for Heun it is the trapezoid
+ * sum -- from the same device reduction as abm_moments.  out[0 .. n_param_sets) (HOST); waits.
+ * ABM_EINVAL before the first step (no time has passed). */
+int abm_time_averaged_velocity(abm_ctx* ctx, double* out);
+
+/* Headless presentation of the current frame.  The paper draws every work
+ * item as one vertex of the shared OpenGL buffer; here the same frame is
+ * rasterised on the device: a 2-D histogram of the points (x mod L, v) -- a point splat with
+ * additive blending -- and, optionally, an RGBA8 image of it.
+ *   dev_counts  DEVICE uint32[height][width], row-major, 4-byte aligned; overwritten.  Column
+ *               ix = position bin over [0, L), row iy = velocity bin over [v_min, v_max), row 0 at v_min.
+ *   dev_rgba    DEVICE uint8[height][width][4] or NULL; grey ramp R = G = B =
+ *               min(255, floor(255 * count / saturation)), A = 255; saturation >= 1.
+ * Bin rule, in IEEE fp64 with every operation rounded on its own (no contraction), on the state
+ * values converted exactly to double:
+ *   xi = x / L;  f = xi - floor(xi);  ix = min(width - 1, floor(f * width))
+ *   eta = (v - v_min) / (v_max - v_min);  the point is dropped unless 0 <= eta < 1;
+ *   iy = min(height - 1, floor(eta * height)).
+ * Non-finite states are dropped.  width * height <= 2^30.  Asynchronous on the context's stream. */
+int abm_raster(abm_ctx* ctx, uint32_t* dev_counts, uint32_t width, uint32_t height, double v_min,
+               double v_max, uint8_t* dev_rgba, uint32_t saturation);
+
 /* Global step count reached so far. */
 int abm_get_step(const abm_ctx* ctx, uint64_t* out_step);
 

@@ -174,3 +174,35 @@ void abo_moments(const double* x, const double* v, const double* e, const double
   out[0] = mx; out[1] = vx / N; out[2] = mv; out[3] = vv / N;
   out[4] = se / N; out[5] = sdx / N; out[6] = sdx2 / N; out[7] = sx2 / N;
 }
+
+/* Headless presentation (the paper draws each work item as a point of the
+ * vertex buffer): 2-D histogram of the points (x mod L, v).  Bin rule as stated in
+ * include/abm.h, one IEEE double operation at a time:
+ *   xi = x / L; f = xi - floor(xi); ix = min(W - 1, floor(f W))
+ *   eta = (v - v_min) / (v_max - v_min); dropped unless 0 <= eta < 1; iy = min(H - 1, floor(eta H))
+ * counts[iy * W + ix] += 1.  counts must be zeroed by the caller. */
+void abo_raster(const double* x, const double* v, uint64_t n, double L, uint32_t W, uint32_t H,
+                double v_min, double v_max, uint32_t* counts) {
+  double v_range = v_max - v_min;
+  for (uint64_t k = 0; k < n; ++k) {
+    double xi = x[k] / L;
+    double f = xi - floor(xi);
+    double eta = (v[k] - v_min) / v_range;
+    if (!(eta >= 0.0) || !(eta < 1.0) || !(f >= 0.0)) continue;
+    double fx = floor(f * (double)W), fy = floor(eta * (double)H);
+    uint32_t ix = fx >= (double)W ? W - 1 : (uint32_t)fx;
+    uint32_t iy = fy >= (double)H ? H - 1 : (uint32_t)fy;
+    counts[(uint64_t)iy * W + ix] += 1u;
+  }
+}
+
+/* Grey ramp of include/abm.h: level = min(255, floor(255 c / saturation)), alpha 255. */
+void abo_colormap(const uint32_t* counts, uint64_t n_bins, uint32_t saturation, uint8_t* rgba) {
+  for (uint64_t b = 0; b < n_bins; ++b) {
+    uint64_t c = counts[b];
+    uint64_t lv = c >= saturation ? 255u : (255u * c) / saturation;
+    rgba[4 * b + 0] = rgba[4 * b + 1] = rgba[4 * b + 2] = (uint8_t)lv;
+    rgba[4 * b + 3] = 255;
+  }
+}
+

@@ -33,6 +33,8 @@
  *   abo_step (Heun) ............ x_n closed form, order-2 convergence, tilt analytic solution
  *   abo_run / abo_init ......... independent numpy restatement at tiny N, split-run invariance
  *   abo_moments ................ numpy mean/var
+ *   abo_raster / abo_colormap .. numpy.histogram2d on points away from bin edges, a hand-counted
+ *                                fixture (tests/golden/raster_small.txt), edge and wrap cases
  * Parity unpinned: the magnitude of the ratchet current <v> (the paper prints no value; its
  * Fig. 2 is not available).
  */
@@ -103,6 +105,12 @@ void abo_run(const abo_params* p, uint64_t seed, uint64_t traj_first, uint64_t t
  * with dx = x - x0. */
 void abo_moments(const double* x, const double* v, const double* e, const double* x0, uint64_t n,
                  double out[8]);
+
+/* Headless presentation: 2-D histogram of (x mod L, v) and its grey-ramp RGBA8 image (include/abm.h
+ * states the bin rule). */
+void abo_raster(const double* x, const double* v, uint64_t n, double L, uint32_t W, uint32_t H,
+                double v_min, double v_max, uint32_t* counts);
+void abo_colormap(const uint32_t* counts, uint64_t n_bins, uint32_t saturation, uint8_t* rgba);
 
 #ifdef __cplusplus
 }

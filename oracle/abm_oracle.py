@@ -70,6 +70,11 @@ def lib():
         L.abo_run.restype = None
         L.abo_moments.argtypes = [dp, dp, dp, dp, C.c_uint64, dp]
         L.abo_moments.restype = None
+        L.abo_raster.argtypes = [dp, dp, C.c_uint64, C.c_double, C.c_uint32, C.c_uint32, C.c_double,
+                                 C.c_double, u32p]
+        L.abo_raster.restype = None
+        L.abo_colormap.argtypes = [u32p, C.c_uint64, C.c_uint32, C.POINTER(C.c_uint8)]
+        L.abo_colormap.restype = None
         _LIB = L
     return _LIB
 
@@ -163,6 +168,23 @@ def moments(x, v, e, x0):
     lib().abo_moments(_dp(x), _dp(v), _dp(e), _dp(x0), x.shape[0], _dp(out))
     names = ["mean_x", "var_x", "mean_v", "var_v", "mean_e", "mean_dx", "mean_dx2", "mean_x2"]
     return dict(zip(names, out.tolist()))
+
+
+def raster(x, v, L, width, height, v_min, v_max):
+    """-> uint32 [height, width] histogram of (x mod L, v)."""
+    x, v = (np.ascontiguousarray(a, np.float64) for a in (x, v))
+    counts = np.zeros((height, width), np.uint32)
+    lib().abo_raster(_dp(x), _dp(v), x.shape[0], float(L), width, height, float(v_min), float(v_max),
+                     counts.ctypes.data_as(C.POINTER(C.c_uint32)))
+    return counts
+
+
+def colormap(counts, saturation):
+    counts = np.ascontiguousarray(counts, np.uint32)
+    rgba = np.zeros(counts.shape + (4,), np.uint8)
+    lib().abo_colormap(counts.ctypes.data_as(C.POINTER(C.c_uint32)), counts.size, int(saturation),
+                       rgba.ctypes.data_as(C.POINTER(C.c_uint8)))
+    return rgba
 
 
 def host_threads():

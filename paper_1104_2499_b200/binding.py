@@ -46,7 +46,7 @@ MOMENT_DTYPE = np.dtype([("n", "<u8"), ("step", "<u8"), ("mean_x", "<f8"), ("var
                          ("mean_dx", "<f8"), ("mean_dx2", "<f8"), ("mean_x2", "<f8")])
 
 EXPORTS = ["abm_create", "abm_step", "abm_snapshot", "abm_snapshot_host", "abm_moments",
-           "abm_moment_sums", "abm_moments_from_sums", "abm_get_step", "abm_get_accuracy", "abm_destroy",
+           "abm_moment_sums", "abm_moments_from_sums", "abm_time_averaged_velocity", "abm_raster", "abm_get_step", "abm_get_accuracy", "abm_destroy",
            "abm_philox_blocks", "abm_strerror", "abm_abi_version"]
 
 _lib = None
@@ -75,6 +75,8 @@ def lib():
         L.abm_moments.argtypes = [vp, vp]
         L.abm_moment_sums.argtypes = [vp, vp]
         L.abm_moments_from_sums.argtypes = [vp, u32, u64, vp]
+        L.abm_time_averaged_velocity.argtypes = [vp, vp]
+        L.abm_raster.argtypes = [vp, vp, u32, u32, C.c_double, C.c_double, vp, u32]
         L.abm_get_step.argtypes = [vp, C.POINTER(u64)]
         L.abm_get_accuracy.argtypes = [vp, C.POINTER(u32)]
         L.abm_destroy.argtypes = [vp]
@@ -154,6 +156,16 @@ def abm_moments_from_sums(sums, step):
     return out
 
 
+def abm_time_averaged_velocity(ctx, n_param_sets):
+    out = np.zeros(n_param_sets, np.float64)
+    _check("abm_time_averaged_velocity", lib().abm_time_averaged_velocity(ctx, out.ctypes.data))
+    return out
+
+
+def abm_raster(ctx, dev_counts, width, height, v_min, v_max, dev_rgba=None, saturation=1):
+    _check("abm_raster", lib().abm_raster(ctx, dev_counts, width, height, v_min, v_max, dev_rgba, saturation))
+
+
 def abm_get_step(ctx):
     n = C.c_uint64()
     _check("abm_get_step", lib().abm_get_step(ctx, C.byref(n)))
@@ -228,6 +240,20 @@ class Ensemble:
 
     def moment_sums(self):
         return abm_moment_sums(self.ctx, self.n_sets)
+
+    def raster(self, width, height, v_min, v_max, saturation=0):
+        """-> (counts int32-viewed uint32 tensor [height, width], rgba uint8 tensor [height, width, 4] or None);
+        device tensors owned by the caller, written on this ensemble's stream."""
+        torch = self._torch
+        with torch.cuda.stream(self.stream):
+            counts = torch.empty((height, width), dtype=torch.int32, device="cuda")
+            rgba = torch.empty((height, width, 4), dtype=torch.uint8, device="cuda") if saturation else None
+        abm_raster(self.ctx, counts.data_ptr(), width, height, v_min, v_max,
+                   rgba.data_ptr() if rgba is not None else None, saturation or 1)
+        return counts, rgba
+
+    def time_averaged_velocity(self):
+        return abm_time_averaged_velocity(self.ctx, self.n_sets)
 
     def state(self):
         """Current (x, v, e) of all trajectories as a float64 numpy array [n_traj, 3] (host)."""

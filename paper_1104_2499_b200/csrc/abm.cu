@@ -489,6 +489,67 @@ int abm_moment_sums(abm_ctx* c, double* out) {
   return ABM_OK;
 }
 
+int abm_raster(abm_ctx* c, uint32_t* dev_counts, uint32_t width, uint32_t height, double v_min,
+               double v_max, uint8_t* dev_rgba, uint32_t saturation) {
+  const int st = check_ctx(c);
+  if (st != ABM_OK) return st;
+  if (!dev_counts || width == 0 || height == 0 || !(v_max > v_min) || !std::isfinite(v_min) ||
+      !std::isfinite(v_max))
+    return ABM_EINVAL;
+  if (static_cast<uint64_t>(width) * height > 0x40000000ull) return ABM_EINVAL;  // 2^30 bins
+  if (reinterpret_cast<uintptr_t>(dev_counts) % 4 != 0) return ABM_EINVAL;
+  if (dev_rgba && (saturation == 0 || reinterpret_cast<uintptr_t>(dev_rgba) % 4 != 0))
+    return ABM_EINVAL;
+  const uint32_t n_bins = width * height;
+  ABM_CK(c, cudaMemsetAsync(dev_counts, 0, sizeof(uint32_t) * n_bins, c->stream));
+  int n_sm = 148;
+  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, c->device);
+  const uint64_t want = (c->n_traj + RASTER_BLOCK - 1) / RASTER_BLOCK;
+  const bool smem = n_bins <= RASTER_SMEM_BINS;
+  // shared-memory path: few, long-lived CTAs (each pays n_bins zeroing + merging); global path: one pass
+  const uint64_t cap = static_cast<uint64_t>(n_sm) * (smem ? 4 : 8);
+  const uint32_t grid = static_cast<uint32_t>(want < cap ? want : cap);
+  const double v_range = v_max - v_min;
+  auto launch = [&](auto real_tag) {
+    using Real = decltype(real_tag);
+    const Real* x = static_cast<const Real*>(c->x);
+    const Real* v = static_cast<const Real*>(c->v);
+    const Coef<Real>* tab = static_cast<const Coef<Real>*>(c->coef_table);
+    if (smem)
+      raster_kernel<Real, true><<<grid, RASTER_BLOCK, sizeof(uint32_t) * n_bins, c->stream>>>(
+          x, v, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range, dev_counts);
+    else
+      raster_kernel<Real, false><<<grid, RASTER_BLOCK, 0, c->stream>>>(
+          x, v, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range, dev_counts);
+  };
+  if (c->precision == ABM_FP32) launch(float{}); else launch(double{});
+  ABM_CK(c, cudaGetLastError());
+  if (dev_rgba) {
+    colormap_kernel<<<(n_bins + 255) / 256, 256, 0, c->stream>>>(dev_counts, n_bins, saturation,
+                                                                 reinterpret_cast<uchar4*>(dev_rgba));
+    ABM_CK(c, cudaGetLastError());
+  }
+  return ABM_OK;
+}
+
+int abm_time_averaged_velocity(abm_ctx* c, double* out) {
+  const int st = check_ctx(c);
+  if (st != ABM_OK) return st;
+  if (!out || c->step == 0) return ABM_EINVAL;
+  std::vector<double> sums;
+  try {
+    sums.resize(static_cast<size_t>(N_SUMS) * c->n_sets);
+  } catch (const std::bad_alloc&) {
+    return ABM_ENOMEM;
+  }
+  const int rc = abm_moment_sums(c, sums.data());
+  if (rc != ABM_OK) return rc;
+  const double t = static_cast<double>(c->step) * c->dt;
+  for (uint32_t s = 0; s < c->n_sets; ++s)
+    out[s] = sums[static_cast<size_t>(s) * N_SUMS + 6] / sums[static_cast<size_t>(s) * N_SUMS] / t;
+  return ABM_OK;
+}
+
 int abm_moments_from_sums(const double* sums, uint32_t n_param_sets, uint64_t step,
                           abm_moment* out_moments) {
   if (!sums || !out_moments || n_param_sets == 0) return ABM_EINVAL;
@@ -547,6 +608,6 @@ const char* abm_strerror(int status) {
   }
 }
 
-uint32_t abm_abi_version(void) { return 2; }
+uint32_t abm_abi_version(void) { return 3; }
 
 }  // extern "C"

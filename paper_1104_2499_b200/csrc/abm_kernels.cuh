@@ -479,6 +479,80 @@ moments_final_kernel(const double* __restrict__ partial, uint32_t n_sets, uint32
 }
 
 // ---------------------------------------------------------------------------------------------
+// Headless presentation: the paper draws every work item as one vertex of
+// the shared buffer; with no graphics API the frame is rasterised here into a
+// 2-D histogram of (x mod L, v) -- a point splat with additive blending -- and colour-mapped to
+// RGBA8.  The bin of a point is decided in fp64 with individually rounded operations (include/abm.h
+// states the rule), so that the CPU oracle takes the same decision bit for bit.
+//
+// Points are unsorted, so every CTA scatters over the whole image: small images (<= RASTER_SMEM_BINS
+// bins) are privatised in shared memory (shared atomics, then one global reduction per CTA and
+// bin); larger ones use fire-and-forget global reductions (RED.ADD), which the 126 MB L2 absorbs
+// (a 1024 x 1024 image is 4 MB).
+// ---------------------------------------------------------------------------------------------
+constexpr int RASTER_BLOCK = 256;
+constexpr uint32_t RASTER_SMEM_BINS = 12288;  // 48 KB of uint32
+
+// -> bin index, or 0xffffffff if the point is outside the velocity window (or not finite)
+__device__ __forceinline__ uint32_t raster_bin(double x, double v, double L, double v_min,
+                                               double v_range, uint32_t W, uint32_t H) {
+  const double xi = __ddiv_rn(x, L);
+  const double f = __dsub_rn(xi, floor(xi));                 // in [0, 1]
+  const double eta = __ddiv_rn(__dsub_rn(v, v_min), v_range);
+  if (!(eta >= 0.0) || !(eta < 1.0) || !(f >= 0.0)) return 0xffffffffu;  // also drops NaN
+  uint32_t ix = static_cast<uint32_t>(floor(__dmul_rn(f, static_cast<double>(W))));
+  uint32_t iy = static_cast<uint32_t>(floor(__dmul_rn(eta, static_cast<double>(H))));
+  if (ix >= W) ix = W - 1;  // f == 1 after rounding (x a hair below a multiple of L)
+  if (iy >= H) iy = H - 1;
+  return iy * W + ix;
+}
+
+template <typename Real, bool SMEM>
+__global__ void __launch_bounds__(RASTER_BLOCK)
+raster_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
+              const Coef<Real>* __restrict__ coef_table, uint64_t n_traj, uint64_t n_particles,
+              uint32_t n_sets, uint32_t W, uint32_t H, double v_min, double v_range,
+              uint32_t* __restrict__ counts) {
+  extern __shared__ uint32_t hist[];
+  const uint32_t n_bins = W * H;
+  if (SMEM) {
+    for (uint32_t b = threadIdx.x; b < n_bins; b += RASTER_BLOCK) hist[b] = 0;
+    __syncthreads();
+  }
+  const uint64_t stride = static_cast<uint64_t>(gridDim.x) * RASTER_BLOCK;
+  for (uint64_t k = static_cast<uint64_t>(blockIdx.x) * RASTER_BLOCK + threadIdx.x; k < n_traj;
+       k += stride) {
+    const uint32_t set = n_sets == 1 ? 0u : static_cast<uint32_t>(k / n_particles);
+    const double L = static_cast<double>(coef_table[set].L);
+    const uint32_t bin = raster_bin(static_cast<double>(x[k]), static_cast<double>(v[k]), L, v_min,
+                                    v_range, W, H);
+    if (bin != 0xffffffffu) {
+      if (SMEM) atomicAdd(&hist[bin], 1u);
+      else atomicAdd(&counts[bin], 1u);  // result unused: compiles to RED.E.ADD
+    }
+  }
+  if (SMEM) {
+    __syncthreads();
+    for (uint32_t b = threadIdx.x; b < n_bins; b += RASTER_BLOCK) {
+      const uint32_t c = hist[b];
+      if (c) atomicAdd(&counts[b], c);
+    }
+  }
+}
+
+// counts -> RGBA8 grey ramp: level = min(255, floor(255 c / saturation)), alpha 255.
+__global__ void __launch_bounds__(256)
+colormap_kernel(const uint32_t* __restrict__ counts, uint32_t n_bins, uint32_t saturation,
+                uchar4* __restrict__ rgba) {
+  const uint32_t b = blockIdx.x * 256u + threadIdx.x;
+  if (b >= n_bins) return;
+  const uint64_t c = counts[b];
+  const uint64_t lv = c >= saturation ? 255ull : (255ull * c) / saturation;
+  const unsigned char l = static_cast<unsigned char>(lv);
+  rgba[b] = make_uchar4(l, l, l, 255);
+}
+
+// ---------------------------------------------------------------------------------------------
 // Diagnostic: raw Philox blocks of the stream
 // ---------------------------------------------------------------------------------------------
 __global__ void philox_blocks_kernel(uint64_t seed, uint64_t traj_first, uint64_t n_traj,

@@ -89,4 +89,18 @@ def config4(n_particles: int = 4_194_304, n_steps: int = 50_000) -> Workload:
                     base=_base(precision=1, dt=1e-4, A1=2.0, A2=0.5, D=0.2, q=1.5, init_v=1))
 
 
+def paper_f0_sweep(n_F0: int = 65_536, F0_min: float = -1.0, F0_max: float = 0.0, realisations: int = 1,
+                   n_steps: int = 10_000, h: float = 1.0, seed: int = 1104) -> Workload:
+    """The paper's own workload: work items that
+    differ only in the load force F0 ("opposing" = negative, reading G13), 2^0 .. 2^16 of them, on the Eq. 3
+    potential of height h (reading G2), run for 10^3..10^4 iterations per launch; the plotted quantity is the
+    mean velocity averaged over time and launches, i.e. <x(t) - x(0)> / t (abm_time_averaged_velocity).
+    The paper prints no parameter values: the depot parameters are those of BASELINE.json configs[0].
+    F0_k = F0_min + (F0_max - F0_min) k / (n_F0 - 1)."""
+    k = np.arange(n_F0, dtype=np.float64)
+    F0 = F0_min + (F0_max - F0_min) * k / max(n_F0 - 1, 1)
+    return Workload(f"paper_f0_sweep_{n_F0}x{realisations}", realisations, n_F0, seed, n_steps,
+                    base=_base(**paper_potential(h)), sweep=dict(F0=F0))
+
+
 CONFIGS = [config0, config1, config2, config3, config4]

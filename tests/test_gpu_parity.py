@@ -374,3 +374,78 @@ def test_gpu_depot_stationary_speed(abm, precision):
     tol = 1e-4 if precision == 0 else 1e-10
     assert st[:, 1]**2 == pytest.approx(1.0 / 1.0 - 0.1 / 1.0, rel=tol)
     assert st[:, 2] == pytest.approx(1.0, rel=tol)
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-3  headless presentation: the rasterised frame is integer work -> bit-exact vs the oracle
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("name,mk,n_particles,n_sets,W_,H_", [
+    ("f32_smem", W.config0, 4096, 1, 96, 64),          # 6,144 bins: shared-memory path
+    ("f32_smem_ragged", W.config0, 1000, 1, 37, 5),
+    ("f32_global", W.config0, 70_001, 1, 1024, 1024),   # global reductions, ragged tail
+    ("f32_sweep", W.config2, 64, 300, 256, 128),        # many sets (same L)
+    ("f64_global", W.config4, 30_000, 1, 640, 480),
+    ("one_bin", W.config0, 513, 1, 1, 1),
+])
+def test_raster_bit_exact(abm, torch, oracle, name, mk, n_particles, n_sets, W_, H_):
+    wl = mk()
+    sets = small(wl, n_particles, n_sets if wl.n_param_sets > 1 else None)
+    with abm.Ensemble(sets, n_particles, wl.seed) as ens:
+        ens.step(203)
+        st = ens.state()
+        v_lo, v_hi = -1.25, 1.5                      # cuts the tails: exercises the dropped points
+        counts, rgba = ens.raster(W_, H_, v_lo, v_hi, saturation=3)
+        torch.cuda.synchronize()
+        counts2, _ = ens.raster(W_, H_, v_lo, v_hi)  # the buffer is re-zeroed on every call
+        torch.cuda.synchronize()
+    got = counts.cpu().numpy().view(np.uint32)
+    want = oracle.raster(st[:, 0], st[:, 1], sets[0]["L"], W_, H_, v_lo, v_hi)
+    assert np.array_equal(got, want)
+    assert np.array_equal(counts2.cpu().numpy().view(np.uint32), want)
+    inside = (st[:, 1] >= v_lo) & (st[:, 1] < v_hi)
+    assert 0 < got.sum() == inside.sum() <= st.shape[0]
+    assert np.array_equal(rgba.cpu().numpy(), oracle.colormap(want, 3))
+
+
+def test_raster_argument_checks(abm, torch):
+    wl = W.config0()
+    with abm.Ensemble([wl.set_params(0)], 64, wl.seed) as ens:
+        buf = torch.zeros(64, dtype=torch.int32, device="cuda")
+        for args in [(None, 8, 8, -1.0, 1.0, None, 1), (buf.data_ptr(), 0, 8, -1.0, 1.0, None, 1),
+                     (buf.data_ptr(), 8, 8, 1.0, 1.0, None, 1), (buf.data_ptr(), 8, 8, -1.0, float("nan"), None, 1),
+                     (buf.data_ptr() + 2, 8, 8, -1.0, 1.0, None, 1),
+                     (buf.data_ptr(), 8, 8, -1.0, 1.0, buf.data_ptr(), 0)]:
+            with pytest.raises(abm.AbmError) as ei:
+                abm.abm_raster(ens.ctx, *args)
+            assert ei.value.status == abm.ABM_EINVAL
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-1  the paper's workload: <v>(F0) as the time- and launch-averaged velocity
+# ---------------------------------------------------------------------------------------------
+
+def test_paper_f0_sweep_time_averaged_velocity(abm, oracle):
+    wl = W.paper_f0_sweep(n_F0=33, F0_min=-3.0, F0_max=3.0, realisations=64, n_steps=400)
+    sets = [wl.set_params(s) for s in range(wl.n_param_sets)]
+    with abm.Ensemble(sets, wl.n_particles, wl.seed) as ens:
+        with pytest.raises(abm.AbmError):
+            ens.time_averaged_velocity()              # no time has passed yet
+        ens.step(150)
+        ens.step(250)                                 # averaged over launches as well
+        vbar = ens.time_averaged_velocity()
+        m = ens.moments()
+        st = ens.state().reshape(wl.n_param_sets, wl.n_particles, 3)
+    t = 400 * sets[0]["dt"]
+    assert np.allclose(vbar, m["mean_dx"] / t, rtol=1e-14, atol=0)
+    for s in (0, 7, 16, 25, 32):
+        first = s * wl.n_particles
+        x, v, e = oracle.init_many(sets[s], wl.seed, wl.n_particles, first)
+        x0 = x.copy()
+        oracle.run(sets[s], wl.seed, x, v, e, 0, 400, first)
+        want = np.mean(x - x0) / t
+        # same trajectories on both sides: fp32 state error only
+        assert abs(vbar[s] - want) <= 1e-4 * max(1.0, abs(want)), (s, vbar[s], want)
+        assert scale_rel_err(st[s], np.stack([x, v, e], 1)).max() <= 1e-4   # 400 steps of error growth
+    # a strong load drags the particle its way (reading G13: +F0 as printed)
+    assert vbar[0] < -0.2 and vbar[-1] > 0.2

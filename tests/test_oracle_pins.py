@@ -496,3 +496,93 @@ def test_config0_orientation_magnitudes(oracle):
     x, v, e = oracle.init_many(p, wl.seed, 1024)
     oracle.run(p, wl.seed, x, v, e, 0, wl.n_steps, threads=oracle.host_threads())
     assert 0.7 < v.var() < 1.4 and 0.8 < e.mean() < 1.1 and np.abs(x).max() < 30
+
+
+# ---- headless presentation ------------------------------------------------
+
+def _load_raster_fixture():
+    pts, rows = [], []
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "raster_small.txt")):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        tok = line.split()
+        if tok[0] == "counts":
+            rows.append([int(t) for t in tok[1:]])
+        else:
+            pts.append((float(tok[0]), float(tok[1])))
+    return np.array(pts), np.array(rows, np.uint32)
+
+
+def test_raster_hand_counted_fixture(oracle):
+    pts, want = _load_raster_fixture()
+    got = oracle.raster(pts[:, 0], pts[:, 1], 1.0, 4, 2, -1.0, 1.0)
+    assert np.array_equal(got, want)
+    assert got.sum() == 6                      # two points fall outside the half-open velocity window
+
+
+@pytest.mark.parametrize("L,W,H", [(1.0, 64, 48), (2.5, 1000, 7), (1.0, 1, 1)])
+def test_raster_matches_numpy_histogram2d(oracle, L, W, H):
+    rng = np.random.default_rng(5)
+    n = 200_000
+    x = rng.normal(0.0, 3.0 * L, n)            # many periods, both signs
+    v = rng.normal(0.0, 1.0, n)
+    v_min, v_max = -2.0, 2.5
+    # keep points clear of bin edges: numpy bins by comparing with linspace edges, the rule divides
+    fx = (x / L - np.floor(x / L)) * W
+    fy = (v - v_min) / (v_max - v_min) * H
+    ok = (np.abs(fx - np.round(fx)) > 1e-6) & (np.abs(fy - np.round(fy)) > 1e-6)
+    x, v = x[ok], v[ok]
+    got = oracle.raster(x, v, L, W, H, v_min, v_max)
+    want, _, _ = np.histogram2d(v, np.mod(x, L), bins=[H, W], range=[[v_min, v_max], [0.0, L]])
+    assert np.array_equal(got, want.astype(np.uint32))
+    inside = (v >= v_min) & (v < v_max)
+    assert got.sum() == inside.sum()
+
+
+def test_raster_edges_and_nonfinite(oracle):
+    x = np.array([0.0, -1e-20, 1.0 - 1e-17, np.nan, 0.5, 0.5, np.inf])
+    v = np.array([0.0, 0.0, 0.0, 0.0, np.nan, 0.9999, 0.0])
+    got = oracle.raster(x, v, 1.0, 8, 4, -1.0, 1.0)
+    # x = -1e-20: xi - floor(xi) rounds to 1 -> last column; 1 - 1e-17 rounds to 1.0 -> f = 0 -> column 0
+    assert got[2, 0] == 2 and got[2, 7] == 1 and got[3, 4] == 1 and got.sum() == 4
+
+
+def test_colormap_ramp(oracle):
+    counts = np.array([[0, 1, 2, 3], [4, 5, 1000, 2**32 - 1]], np.uint32)
+    rgba = oracle.colormap(counts, 4)
+    assert rgba.shape == (2, 4, 4) and np.all(rgba[..., 3] == 255)
+    assert np.array_equal(rgba[..., 0], np.minimum(255, (255 * counts.astype(np.uint64)) // 4).astype(np.uint8))
+    assert np.array_equal(rgba[..., 0], rgba[..., 1]) and np.array_equal(rgba[..., 0], rgba[..., 2])
+    assert np.array_equal(oracle.colormap(counts, 1)[..., 0], np.where(counts > 0, 255, 0))
+
+
+# ---- the paper's own workload: <v>(F0) -------------------------------------
+
+def test_time_averaged_velocity_of_a_loaded_free_particle(oracle):
+    """D = 0, no potential: the time average <x(t) - x(0)> / t converges to the stationary speed, the root of
+    F0 + d e v - gamma0 v = 0 with e = q / (c + d v^2) (Eqs. 1-2 at rest); the sign of F0 selects the branch
+    (reading G13: +F0 as printed)."""
+    from scipy.optimize import brentq
+    base = dict(W.DEFAULTS, A1=0.0, A2=0.0, D=0.0, v0=0.0, e0=0.0, dt=1e-3)
+    for F0 in (-0.5, 0.3):
+        p = dict(base, F0=F0)
+        g = lambda vv: F0 + p["d"] * p["q"] / (p["c"] + p["d"] * vv * vv) * vv - p["gamma0"] * vv
+        root = brentq(g, 0.5 * np.sign(F0), 3.0 * np.sign(F0))
+        x, v, e = oracle.init_many(p, 3, 4)
+        x0 = x.copy()
+        n = 200_000
+        oracle.run(p, 3, x, v, e, 0, n)
+        assert np.allclose(v, root, rtol=1e-6)
+        vbar = (x - x0) / (n * p["dt"])
+        assert np.allclose(vbar, root, rtol=2e-2)           # transient of a few time units out of 200
+        assert np.sign(vbar[0]) == np.sign(F0)
+
+
+def test_paper_f0_sweep_workload_shape():
+    wl = W.paper_f0_sweep(n_F0=17, F0_min=-1.0, F0_max=0.0, realisations=3, n_steps=100)
+    assert wl.n_param_sets == 17 and wl.n_particles == 3 and wl.n_trajectories == 51
+    f = [wl.set_params(s)["F0"] for s in range(17)]
+    assert f[0] == -1.0 and f[-1] == 0.0 and np.allclose(np.diff(f), 1 / 16)
+    p = wl.set_params(5)
+    assert p["phi"] == 0.1903 and p["A1"] == -0.453 and p["A2"] == -0.11325 and p["L"] == 1.0
