@@ -9,11 +9,11 @@ namespace abm {
 #define ABM_STEP_BLOCK 128
 #endif
 // Resident CTAs per SM of the step kernel (the register cap follows: 65,536 / (128 * n)), per
-// kernel family.  The loop is bound by the FMA dispatch port, not by latency, so 6-8 warps per
-// scheduler are enough; what matters is (i) no spills in the loop and (ii) little wave
-// quantisation: all CTAs run equally long, so T / (148 * 128 * n) waves round UP
-// (config[1]: n = 12 -> 4.61 waves cost 5; n = 8 -> 6.92 cost 7).
-// Measured on B200 (steady state, round-1 sweeps): fp32 EM one set 8 > 7 > 6 > 12;
+// kernel family.  The loop is throughput-bound from four warps per scheduler on
+// (profiles/r01_scaling.md: no wave quantisation, a partly filled wave runs proportionally
+// faster), so occupancy is chosen for the code ptxas produces under the cap -- no spills, few
+// moves -- not for latency hiding.
+// Measured on B200 (round-1 sweeps, particle-steps/s): fp32 EM one set 8 > 7 > 5 > 6 > 12;
 // fp32 Heun 5 ~ 4 > 6 > 8; fp32 with per-thread coefficients 4 > 6 > 8 > 12 (12 spilled 236 B);
 // fp64 insensitive between 4 and 8 (12 spilled > 1 KB).
 #ifndef ABM_MINB_F32U
