@@ -35,8 +35,11 @@ from paper_1104_2499_b200 import workloads as W  # noqa: E402
 
 # Algorithmic (necessary) warp-lane instructions per particle-step, frozen in BASELINE.md /
 # DESIGN.md before tuning.
-I_ALG = {0: 29.0, 1: 29.0, 2: 29.0, 3: 45.0, 4: 110.0}
+I_ALG = {0: 29.0, 1: 29.0, 2: 29.0, 3: 45.0, 4: 60.0}
 N_SM, LANES_PER_SM = 148, 128
+# config[4] is bound by the FP64 pipe (64 lanes/clk/SM; 59 measured for DFMA), not by issue slots: its
+# I_alg counts the ~60 DFMA-pipe operations per particle-step and its peak is 64 lanes.
+LANES_FP64 = 64
 
 
 def load_peaks():
@@ -314,19 +317,21 @@ def run_ours(args, wl, cfg_id):
     if t_kern_ms:
         t_k = statistics.mean(t_kern_ms) * 1e-3
         lane_instr = I_ALG[cfg_id] * wl.particle_steps
-        peak = N_SM * LANES_PER_SM * f_max
+        lanes = LANES_FP64 if fp64 else LANES_PER_SM
+        peak = N_SM * lanes * f_max
         achieved = lane_instr / t_k
         sm_mhz = clocks.get("sm_mhz") or (f_max / 1e6)
         out["roofline"] = {
             "bound": "alu", "kernel": "abm::step_kernel", "achieved": achieved / 1e12,
-            "peak": peak / 1e12, "unit": "Tinstr/s (warp-lane instructions)",
+            "peak": peak / 1e12,
+            "unit": "Tinstr/s (FP64-pipe lane operations)" if fp64 else "Tinstr/s (warp-lane instructions)",
             "frac": achieved / peak,
-            "frac_at_sustained_clock": achieved / (N_SM * LANES_PER_SM * sm_mhz * 1e6),
+            "frac_at_sustained_clock": achieved / (N_SM * lanes * sm_mhz * 1e6),
             "i_alg_per_particle_step": I_ALG[cfg_id],
             "particle_steps_per_pass": wl.particle_steps,
             "kernel_ms": 1e3 * t_k, "kernel_launches_per_pass": step_launches * (n_steps // M),
             "kernel_share_of_pass": sum(t_kern_ms) / sum(t_pass_ms),
-            "peak_source": f"148 SMs x 128 lanes x sm_max_mhz {f_max / 1e6:.0f} MHz, {peak_src}",
+            "peak_source": f"148 SMs x {lanes} lanes x sm_max_mhz {f_max / 1e6:.0f} MHz, {peak_src}",
             "traffic": None,
             "hbm_algorithmic_bytes_per_launch": int(T * (24 + 8 * (n_steps // wl.snapshot_every
                                                                    if wl.snapshot_every else 0))),
