@@ -136,14 +136,20 @@ def abm_snapshot_host(ctx, host_array, stride_bytes):
     _check("abm_snapshot_host", lib().abm_snapshot_host(ctx, host_array.ctypes.data, stride_bytes))
 
 
-def abm_moments(ctx, n_param_sets):
-    out = np.zeros(n_param_sets, MOMENT_DTYPE)
+def abm_moments(ctx, n_param_sets, out=None):
+    """`out`: optional caller-owned record array [n_param_sets] (e.g. a view of pinned host memory, which
+    makes the device->host copy a true DMA); a fresh pageable array otherwise."""
+    if out is None:
+        out = np.zeros(n_param_sets, MOMENT_DTYPE)
+    assert out.dtype == MOMENT_DTYPE and out.shape == (n_param_sets,) and out.flags.c_contiguous
     _check("abm_moments", lib().abm_moments(ctx, out.ctypes.data))
     return out
 
 
-def abm_moment_sums(ctx, n_param_sets):
-    out = np.zeros((n_param_sets, ABM_N_SUMS), np.float64)
+def abm_moment_sums(ctx, n_param_sets, out=None):
+    if out is None:
+        out = np.zeros((n_param_sets, ABM_N_SUMS), np.float64)
+    assert out.dtype == np.float64 and out.shape == (n_param_sets, ABM_N_SUMS) and out.flags.c_contiguous
     _check("abm_moment_sums", lib().abm_moment_sums(ctx, out.ctypes.data))
     return out
 
@@ -186,6 +192,17 @@ def abm_philox_blocks(seed, traj_first, n_traj, block_first, n_blocks, dev_ptr, 
     _check("abm_philox_blocks",
            lib().abm_philox_blocks(seed, traj_first, n_traj, block_first & 0xffffffffffffffff,
                                    n_blocks, dev_ptr, stream or None))
+
+
+def pinned_moment_buffers(n_param_sets):
+    """(records, sums) numpy views of pinned host memory (torch owns it) for abm_moments / abm_moment_sums."""
+    import torch
+    rec = torch.zeros(n_param_sets * MOMENT_DTYPE.itemsize, dtype=torch.uint8, pin_memory=True)
+    sums = torch.zeros((n_param_sets, ABM_N_SUMS), dtype=torch.float64, pin_memory=True)
+    out = rec.numpy().view(MOMENT_DTYPE)
+    out_s = sums.numpy()
+    out.flags.writeable = True
+    return (out, rec), (out_s, sums)
 
 
 # ---- convenience wrapper (owns the handle and the torch snapshot buffer) ----------------------
@@ -235,11 +252,11 @@ class Ensemble:
     def step(self, n):
         abm_step(self.ctx, n)
 
-    def moments(self):
-        return abm_moments(self.ctx, self.n_sets)
+    def moments(self, out=None):
+        return abm_moments(self.ctx, self.n_sets, out)
 
-    def moment_sums(self):
-        return abm_moment_sums(self.ctx, self.n_sets)
+    def moment_sums(self, out=None):
+        return abm_moment_sums(self.ctx, self.n_sets, out)
 
     def raster(self, width, height, v_min, v_max, saturation=0):
         """-> (counts int32-viewed uint32 tensor [height, width], rgba uint8 tensor [height, width, 4] or None);

@@ -20,7 +20,7 @@ DEPS = SOURCES + [os.path.join(CSRC, "abm_device.cuh"), os.path.join(CSRC, "abm_
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "-Xcompiler", "-fPIC", "-Xcompiler", "-pthread", "-shared", "-cudart", "static",
     "-I", os.path.join(ROOT, "include"), "-I", CSRC,
 ]
 

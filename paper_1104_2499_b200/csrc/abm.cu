@@ -11,6 +11,7 @@
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <thread>
 #include <vector>
 
 #include "abm_kernels.cuh"
@@ -200,13 +201,41 @@ void free_all(abm_ctx* c) {
   c->host_coefs = nullptr;
 }
 
+// Host loops over parameter sets (coefficient precomputation): a sweep has up to 2^16 sets and the
+// device idles meanwhile, so large tables are split over a few host threads.
+template <typename F>
+void parallel_sets(uint32_t n_sets, F&& body) {
+  unsigned n_thr = std::thread::hardware_concurrency();
+  if (n_thr > 8) n_thr = 8;
+  if (n_sets < 8192 || n_thr < 2) {
+    body(0u, n_sets);
+    return;
+  }
+  std::vector<std::thread> pool;
+  const uint32_t chunk = (n_sets + n_thr - 1) / n_thr;
+  try {
+    for (uint32_t s0 = chunk; s0 < n_sets; s0 += chunk)
+      pool.emplace_back([&body, s0, chunk, n_sets] { body(s0, s0 + chunk < n_sets ? s0 + chunk : n_sets); });
+  } catch (...) {  // could not start (more) threads: the rest runs here
+    const uint32_t started = static_cast<uint32_t>(pool.size());
+    for (auto& t : pool) t.join();
+    body(0u, chunk < n_sets ? chunk : n_sets);
+    if ((started + 1) * chunk < n_sets) body((started + 1) * chunk, n_sets);
+    return;
+  }
+  body(0u, chunk < n_sets ? chunk : n_sets);
+  for (auto& t : pool) t.join();
+}
+
 template <typename Real>
 int upload_coefs_and_init(abm_ctx* c, const abm_params* params) {
   // the host copy lives as long as the context: the upload is asynchronous
   Coef<Real>* tab = static_cast<Coef<Real>*>(std::malloc(sizeof(Coef<Real>) * c->n_sets));
   if (!tab) return ABM_ENOMEM;
   c->host_coefs = tab;
-  for (uint32_t s = 0; s < c->n_sets; ++s) tab[s] = make_coef<Real>(params[s]);
+  parallel_sets(c->n_sets, [&](uint32_t s0, uint32_t s1) {
+    for (uint32_t s = s0; s < s1; ++s) tab[s] = make_coef<Real>(params[s]);
+  });
   ABM_CK(c, dev_alloc(c, &c->coef_table, sizeof(Coef<Real>) * c->n_sets));
   ABM_CK(c, cudaMemcpyAsync(c->coef_table, tab, sizeof(Coef<Real>) * c->n_sets,
                             cudaMemcpyHostToDevice, c->stream));
