@@ -68,6 +68,37 @@ void abo_normals(uint64_t seed, uint64_t traj_first, uint64_t n_traj, uint64_t s
       out[k * n_steps + j] = abo_normal(seed, traj_first + k, step_first + j, precision);
 }
 
+/* ---- NEXT-4: the paper's generator family -------------------------------------- */
+
+uint32_t abo_xorshift128(uint32_t s[4]) {
+  uint32_t t = s[0] ^ (s[0] << 11);
+  s[0] = s[1]; s[1] = s[2]; s[2] = s[3];
+  s[3] = s[3] ^ (s[3] >> 19) ^ t ^ (t >> 8);
+  return s[3];
+}
+
+void abo_xorshift_seed(uint64_t seed, uint64_t traj, uint32_t s[4]) {
+  abo_block(seed, traj, UINT64_MAX - 1u, s);
+  if ((s[0] | s[1] | s[2] | s[3]) == 0u) s[3] = 1u; /* the one forbidden state */
+}
+
+static double normal_from_pair(uint32_t a, uint32_t b, uint64_t n, int32_t precision) {
+  double u1 = abo_uniform(a, precision);
+  double u2 = abo_uniform(b, precision);
+  double r = sqrt(-2.0 * log(u1));
+  if ((n & 1u) == 0) return r * cos(ABO_TWO_PI * u2);
+  return r * sin(ABO_TWO_PI * u2);
+}
+
+double abo_normal_xorshift(uint64_t seed, uint64_t traj, uint64_t n, int32_t precision) {
+  uint32_t s[4];
+  abo_xorshift_seed(seed, traj, s);
+  for (uint64_t j = 0; j < 2u * (n >> 1); ++j) (void)abo_xorshift128(s); /* outputs of earlier pairs */
+  uint32_t a = abo_xorshift128(s);
+  uint32_t b = abo_xorshift128(s);
+  return normal_from_pair(a, b, n, precision);
+}
+
 /* ---- 8(c)-6: right-hand side (Eqs. 1-3) --------------------------------------------------- */
 
 double abo_potential(const abo_params* p, double x) {
@@ -106,12 +137,11 @@ void abo_init(const abo_params* p, uint64_t seed, uint64_t traj, double* x, doub
 
 /* ---- 8(c)-7/8: one step ------------------------------------------------------------------- */
 
-void abo_step(const abo_params* p, uint64_t seed, uint64_t traj, uint64_t n, double* x, double* v,
-              double* e) {
+static void step_with_normal(const abo_params* p, uint64_t n, double z, double* x, double* v,
+                             double* e) {
   double dt = p->dt;
   double t_n = (double)n * dt;
   double sigma = sqrt(2.0 * p->D * dt);
-  double z = abo_normal(seed, traj, n, p->precision);
   double ax, av, ae;
   abo_rhs(p, *x, *v, *e, t_n, &ax, &av, &ae);
   if (p->integrator == 0) {
@@ -136,6 +166,13 @@ void abo_step(const abo_params* p, uint64_t seed, uint64_t traj, uint64_t n, dou
   }
 }
 
+void abo_step(const abo_params* p, uint64_t seed, uint64_t traj, uint64_t n, double* x, double* v,
+              double* e) {
+  double z = p->rng == 0 ? abo_normal(seed, traj, n, p->precision)
+                         : abo_normal_xorshift(seed, traj, n, p->precision);
+  step_with_normal(p, n, z, x, v, e);
+}
+
 /* ---- ensembles ----------------------------------------------------------------------------- */
 
 void abo_init_many(const abo_params* p, uint64_t seed, uint64_t traj_first, uint64_t traj_stride,
@@ -149,8 +186,25 @@ void abo_run(const abo_params* p, uint64_t seed, uint64_t traj_first, uint64_t t
              double* e) {
   for (uint64_t k = 0; k < n_traj; ++k) {
     uint64_t traj = traj_first + k * traj_stride;
-    for (uint64_t n = step_first; n < step_first + n_steps; ++n)
-      abo_step(p, seed, traj, n, &x[k], &v[k], &e[k]);
+    if (p->rng == 0) {
+      for (uint64_t n = step_first; n < step_first + n_steps; ++n)
+        abo_step(p, seed, traj, n, &x[k], &v[k], &e[k]);
+    } else {
+      /* xorshift mode: the same steps with the generator carried along instead of re-run from its
+       * seed at every step (abo_step does that; tests check the two agree). */
+      uint32_t s[4], a = 0, b = 0;
+      abo_xorshift_seed(seed, traj, s);
+      for (uint64_t j = 0; j < 2u * (step_first >> 1); ++j) (void)abo_xorshift128(s);
+      int have_pair = 0;
+      for (uint64_t n = step_first; n < step_first + n_steps; ++n) {
+        if (!have_pair || (n & 1u) == 0) {
+          a = abo_xorshift128(s);
+          b = abo_xorshift128(s);
+          have_pair = 1;
+        }
+        step_with_normal(p, n, normal_from_pair(a, b, n, p->precision), &x[k], &v[k], &e[k]);
+      }
+    }
   }
 }
 

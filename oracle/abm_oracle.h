@@ -33,6 +33,8 @@
  *   abo_step (Heun) ............ x_n closed form, order-2 convergence, tilt analytic solution
  *   abo_run / abo_init ......... independent numpy restatement at tiny N, split-run invariance
  *   abo_moments ................ numpy mean/var
+ *   abo_xorshift128 ............ Marsaglia (2003) xor128 first outputs from the paper's default state
+ *                                (tests/golden/xorshift128_kat.txt), invertibility, normal moments
  *   abo_raster / abo_colormap .. numpy.histogram2d on points away from bin edges, a hand-counted
  *                                fixture (tests/golden/raster_small.txt), edge and wrap cases
  * Parity unpinned: the magnitude of the ratchet current <v> (the paper prints no value; its
@@ -51,7 +53,8 @@ typedef struct abo_params {
   int32_t precision;  /* 0: run uses the fp32 uniform maps; 1: the fp64 maps          */
   int32_t integrator; /* 0: Euler-Maruyama; 1: stochastic Heun                         */
   int32_t init_v;     /* 0: v(0) = v0; 1: v(0) ~ N(0, D/gamma0) from the init block    */
-  int32_t reserved;
+  int32_t rng;        /* 0: Philox4x32-10 stream (BASELINE.json); 1: per-trajectory Marsaglia
+                         xorshift state as in the paper   */
   double dt;
   double gamma0, q, c, d, D; /* Eqs. 1-2 */
   double F0;                 /* constant load force, enters as +F0 (reading G13)       */
@@ -79,6 +82,17 @@ double abo_normal(uint64_t seed, uint64_t traj, uint64_t n, int32_t precision);
  * step_first + j (a plain double loop over abo_normal). */
 void abo_normals(uint64_t seed, uint64_t traj_first, uint64_t n_traj, uint64_t step_first,
                  uint64_t n_steps, int32_t precision, double* out);
+
+/* NEXT-4 generator variant ("Marsaglia xor-shift algorithm"; the exact variant is not
+ * printed -- reading: xor128 of G. Marsaglia, "Xorshift RNGs", J. Stat. Softw. 8(14), 2003, p. 5:
+ * t = x ^ (x << 11); x = y; y = z; z = w; w = w ^ (w >> 19) ^ t ^ (t >> 8); return w).
+ * One state (x, y, z, w) per trajectory, seeded from the Philox block b = 2^64 - 2 of the trajectory
+ * (all-zero is replaced by (0, 0, 0, 1)).  Output j (0-based) of the trajectory's generator feeds:
+ * pair p = n >> 1 of steps uses u1 = u(output 2p), u2 = u(output 2p + 1); normals as for Philox. */
+uint32_t abo_xorshift128(uint32_t s[4]);
+void abo_xorshift_seed(uint64_t seed, uint64_t traj, uint32_t s[4]);
+/* Normal of step n in xorshift mode, by iterating the generator from its seed (O(n): tests only). */
+double abo_normal_xorshift(uint64_t seed, uint64_t traj, uint64_t n, int32_t precision);
 
 /* U(x) without the additive constant, and the right-hand side of Eqs. 1-2 at (x,v,e,t). */
 double abo_potential(const abo_params* p, double x);

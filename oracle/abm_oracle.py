@@ -18,14 +18,14 @@ _LIB = None
 class Params(C.Structure):
     """Mirror of `abo_params` (oracle/abm_oracle.h)."""
     _fields_ = [("precision", C.c_int32), ("integrator", C.c_int32), ("init_v", C.c_int32),
-                ("reserved", C.c_int32),
+                ("rng", C.c_int32),
                 ("dt", C.c_double), ("gamma0", C.c_double), ("q", C.c_double), ("c", C.c_double),
                 ("d", C.c_double), ("D", C.c_double), ("F0", C.c_double), ("A", C.c_double),
                 ("omega", C.c_double), ("L", C.c_double), ("A1", C.c_double), ("A2", C.c_double),
                 ("phi", C.c_double), ("v0", C.c_double), ("e0", C.c_double)]
 
 
-_FIELDS = [f[0] for f in Params._fields_ if f[0] != "reserved"]
+_FIELDS = [f[0] for f in Params._fields_]
 
 
 def make_params(cfg: dict) -> Params:
@@ -70,6 +70,12 @@ def lib():
         L.abo_run.restype = None
         L.abo_moments.argtypes = [dp, dp, dp, dp, C.c_uint64, dp]
         L.abo_moments.restype = None
+        L.abo_xorshift128.argtypes = [u32p]
+        L.abo_xorshift128.restype = C.c_uint32
+        L.abo_xorshift_seed.argtypes = [C.c_uint64, C.c_uint64, u32p]
+        L.abo_xorshift_seed.restype = None
+        L.abo_normal_xorshift.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, C.c_int32]
+        L.abo_normal_xorshift.restype = C.c_double
         L.abo_raster.argtypes = [dp, dp, C.c_uint64, C.c_double, C.c_uint32, C.c_uint32, C.c_double,
                                  C.c_double, u32p]
         L.abo_raster.restype = None
@@ -168,6 +174,23 @@ def moments(x, v, e, x0):
     lib().abo_moments(_dp(x), _dp(v), _dp(e), _dp(x0), x.shape[0], _dp(out))
     names = ["mean_x", "var_x", "mean_v", "var_v", "mean_e", "mean_dx", "mean_dx2", "mean_x2"]
     return dict(zip(names, out.tolist()))
+
+
+def xorshift128(state):
+    """state: 4 uint32 (x, y, z, w) -> (output, new state)"""
+    s = (C.c_uint32 * 4)(*[int(t) for t in state])
+    out = lib().abo_xorshift128(s)
+    return int(out), [int(t) for t in s]
+
+
+def xorshift_seed(seed, traj):
+    s = (C.c_uint32 * 4)()
+    lib().abo_xorshift_seed(seed, traj, s)
+    return [int(t) for t in s]
+
+
+def normal_xorshift(seed, traj, n, precision):
+    return lib().abo_normal_xorshift(seed, traj, n, int(precision))
 
 
 def raster(x, v, L, width, height, v_min, v_max):

@@ -586,3 +586,105 @@ def test_paper_f0_sweep_workload_shape():
     assert f[0] == -1.0 and f[-1] == 0.0 and np.allclose(np.diff(f), 1 / 16)
     p = wl.set_params(5)
     assert p["phi"] == 0.1903 and p["A1"] == -0.453 and p["A2"] == -0.11325 and p["L"] == 1.0
+
+
+# ---- NEXT-4: the paper's generator family --------------------------------------------
+
+def test_xorshift128_known_answers(oracle):
+    state, outs = None, []
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "xorshift128_kat.txt")):
+        tok = line.split("#")[0].split()
+        if tok and tok[0] == "state":
+            state = [int(t) for t in tok[1:]]
+        elif tok and tok[0] == "out":
+            outs.append(int(tok[1]))
+    assert len(outs) == 5
+    for want in outs:
+        got, state = oracle.xorshift128(state)
+        assert got == want and state[3] == want
+
+
+def test_xorshift128_python_restatement_and_bijectivity(oracle):
+    rng = np.random.default_rng(11)
+    seen = set()
+    for _ in range(200):
+        s = [int(t) for t in rng.integers(0, 2**32, 4)]
+        x, y, z, w = s
+        t = (x ^ (x << 11)) & 0xffffffff
+        want = [y, z, w, (w ^ (w >> 19) ^ t ^ (t >> 8)) & 0xffffffff]
+        out, new = oracle.xorshift128(s)
+        assert new == want and out == want[3]
+        seen.add(tuple(new))
+    assert len(seen) == 200
+    # the transition is linear over GF(2): T(a ^ b) = T(a) ^ T(b), and T(0) = 0 (the forbidden state)
+    a = [int(t) for t in rng.integers(0, 2**32, 4)]
+    b = [int(t) for t in rng.integers(0, 2**32, 4)]
+    ta, tb = oracle.xorshift128(a)[1], oracle.xorshift128(b)[1]
+    tab = oracle.xorshift128([p ^ q for p, q in zip(a, b)])[1]
+    assert tab == [p ^ q for p, q in zip(ta, tb)]
+    assert oracle.xorshift128([0, 0, 0, 0]) == (0, [0, 0, 0, 0])
+
+
+def test_xorshift_seed_and_stream_layout(oracle):
+    seed, traj = 0x1234_5678_9abc_def0, 77
+    s = oracle.xorshift_seed(seed, traj)
+    assert s == [int(t) for t in oracle.block(seed, traj, 2**64 - 2)] and any(s)
+    # pair p of steps (2p, 2p + 1) uses outputs 2p and 2p + 1
+    outs = []
+    for _ in range(6):
+        o, s = oracle.xorshift128(s)
+        outs.append(o)
+    for n in range(6):
+        a, b = outs[2 * (n // 2)], outs[2 * (n // 2) + 1]
+        for prec in (0, 1):
+            u1, u2 = oracle.uniform(a, prec), oracle.uniform(b, prec)
+            r = math.sqrt(-2.0 * math.log(u1))
+            want = r * (math.cos(2 * math.pi * u2) if n % 2 == 0 else math.sin(2 * math.pi * u2))
+            assert oracle.normal_xorshift(seed, traj, n, prec) == pytest.approx(want, rel=1e-14, abs=1e-15)
+
+
+def test_xorshift_normals_moments(oracle):
+    """Normals of the xorshift stream over many trajectories and steps: mean 0, variance 1, kurtosis 3."""
+    p = dict(W.DEFAULTS, rng=1, A1=0.0, A2=0.0, d=0.0, q=0.0, c=0.0, gamma0=1.0 / 2.0**-10, dt=2.0**-10,
+             D=0.5 / 2.0**-10)                      # EM: v_{n+1} = z_n exactly (sigma = 1)
+    n_traj, zs = 20_000, []
+    x, v, e = oracle.init_many(p, 5, n_traj)
+    for n in range(24):
+        oracle.run(p, 5, x, v, e, n, 1, threads=8)
+        zs.append(v.copy())
+    z = np.concatenate(zs)
+    N = z.size
+    assert abs(z.mean()) < 3 / math.sqrt(N)
+    assert abs(z.var() - 1) < 3 * math.sqrt(2 / N)
+    assert abs(np.mean(z**4) - 3) < 3 * math.sqrt(96 / N)
+    # consecutive steps (cos / sin of one pair, then the next pair) are uncorrelated
+    zz = np.stack(zs)
+    for lag in (1, 2):
+        c = np.mean(zz[:-lag] * zz[lag:])
+        assert abs(c) < 4 / math.sqrt(zz[:-lag].size)
+    # and the first steps equal the definition evaluated from the seed
+    assert zs[3][17] == oracle.normal_xorshift(5, 17, 3, 0)
+
+
+def test_xorshift_run_matches_stepwise_definition_and_splits(oracle):
+    p = dict(W.config3().set_params(0), rng=1)
+    seed, n = 99, 6
+    x, v, e = oracle.init_many(p, seed, n, 40)
+    x1, v1, e1 = x.copy(), v.copy(), e.copy()
+    x2, v2, e2 = x.copy(), v.copy(), e.copy()
+    oracle.run(p, seed, x, v, e, 0, 23, 40)
+    for a, b in ((0, 5), (5, 1), (6, 7), (13, 10)):         # odd and even split points
+        oracle.run(p, seed, x1, v1, e1, a, b, 40)
+    assert np.array_equal(x, x1) and np.array_equal(v, v1) and np.array_equal(e, e1)
+    L = oracle.lib()
+    pp = oracle.make_params(p)
+    import ctypes as C
+    for k in range(n):
+        xs, vs, es = (C.c_double(t[k]) for t in (x2, v2, e2))
+        for step in range(23):
+            L.abo_step(C.byref(pp), seed, 40 + k, step, C.byref(xs), C.byref(vs), C.byref(es))
+        assert (xs.value, vs.value, es.value) == (x[k], v[k], e[k])
+    # a different stream from the Philox one, same physics
+    xp, vp, ep = oracle.init_many(dict(p, rng=0), seed, n, 40)
+    oracle.run(dict(p, rng=0), seed, xp, vp, ep, 0, 23, 40)
+    assert not np.array_equal(v, vp)
