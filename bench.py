@@ -195,7 +195,7 @@ def run_ours(args, wl, cfg_id):
     abm.lib()
 
     stream = torch.cuda.Stream()
-    sets = [wl.set_params(s) for s in range(wl.n_param_sets)]
+    sets = [dict(wl.set_params(s), rng=1 if args.rng == "xorshift" else 0) for s in range(wl.n_param_sets)]
     T = wl.n_trajectories
     # weak scaling: rank r integrates a full copy of the workload on global trajectories [r*T, (r+1)*T)
     plan = sharding.shard_plan(wl.n_particles, wl.n_param_sets, rank, world, "weak")
@@ -303,7 +303,7 @@ def run_ours(args, wl, cfg_id):
         "config": {"workload": wl.name, "baseline_config": cfg_id, "trajectories_per_gpu": T,
                    "param_sets": wl.n_param_sets, "sim_steps": n_steps,
                    "snapshot_every": wl.snapshot_every, "moments_every": M,
-                   "integrator": "heun" if sets[0]["integrator"] else "euler-maruyama",
+                   "integrator": "heun" if sets[0]["integrator"] else "euler-maruyama", "rng": args.rng,
                    "l2": "flushed between timed iterations (256 MiB fill)",
                    "pass": "create+init, bind frame, integrate, moments, destroy"},
         "e2e": {"value": psteps_job / t_e2e, "unit": "particle-steps/s",
@@ -356,6 +356,8 @@ def main():
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--rng", default="philox", choices=["philox", "xorshift"],
+                    help="generator A/B (SURVEY.md 8(f) NEXT-4); the headline and the roofline are Philox")
     ap.add_argument("--sim-steps", type=int, default=0, help="override the config's step count")
     args = ap.parse_args()
     wl = W.CONFIGS[args.config]()

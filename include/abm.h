@@ -73,6 +73,17 @@ enum { ABM_INIT_V_CONST = 0, ABM_INIT_V_THERMAL = 1 }; /* abm_params.init_v */
  * Ignored in fp64.  Both modes consume the same random stream. */
 enum { ABM_ACCURACY_AUTO = 0, ABM_ACCURACY_FAST = 1, ABM_ACCURACY_PRECISE = 2 };
 
+/* abm_params.rng -- where the uniform words come from.
+ *   PHILOX        counter-based Philox4x32-10 keyed by (seed, trajectory, step): BASELINE.json
+ *                 north_star (b); the stream of DESIGN.md "Random stream".  Default.
+ *   XORSHIFT128   the paper's generator family ("Marsaglia xor-shift"; the variant is not
+ *                 printed -- reading: xor128 of Marsaglia 2003): one state (x, y, z, w) per
+ *                 trajectory, kept in device memory between launches, seeded from Philox block
+ *                 2^64 - 2 of the trajectory; steps (2p, 2p + 1) use outputs 2p and 2p + 1.  For the
+ *                 A/B of generator cost.  Everything else -- initial state,
+ *                 uniform maps, Box-Muller, split-launch bit-identity -- is unchanged. */
+enum { ABM_RNG_PHILOX = 0, ABM_RNG_XORSHIFT128 = 1 };
+
 typedef struct abm_ctx abm_ctx; /* opaque, owned by the library */
 
 /* One record per parameter set (the paper's per-work-item parameter record).
@@ -84,7 +95,9 @@ typedef struct abm_params {
   uint32_t init_v;         /* RC  v(0) = v0, or v(0) ~ N(0, D/gamma0) from the init block      */
   uint32_t snapshot_every; /* RC  K: abm_step rewrites the bound snapshot buffer after every
                                   global step count that is a multiple of K; 0 = never         */
-  uint32_t accuracy;       /* RC  fp32 only: ABM_ACCURACY_AUTO | _FAST | _PRECISE (see below)      */
+  uint32_t accuracy;       /* RC  fp32 only: ABM_ACCURACY_AUTO | _FAST | _PRECISE (see above)      */
+  uint32_t rng;            /* RC  ABM_RNG_PHILOX | ABM_RNG_XORSHIFT128                          */
+  uint32_t reserved;       /*     must be 0                                                    */
   double dt;               /* RC  time step                                                    */
   double gamma0, q, c, d, D; /*   Eqs. 1-2                                                     */
   double F0;               /*     constant load force, +F0 as printed in Eq. 2   */

@@ -17,6 +17,7 @@ ABM_OK, ABM_EINVAL, ABM_ENOMEM, ABM_ECUDA, ABM_ESTATE = 0, -1, -2, -3, -4
 ABM_FP32, ABM_FP64 = 0, 1
 ABM_EULER_MARUYAMA, ABM_HEUN = 0, 1
 ABM_ACCURACY_AUTO, ABM_ACCURACY_FAST, ABM_ACCURACY_PRECISE = 0, 1, 2
+ABM_RNG_PHILOX, ABM_RNG_XORSHIFT128 = 0, 1
 ABM_N_SUMS = 8
 
 
@@ -25,6 +26,7 @@ class abm_params(C.Structure):
     _fields_ = [
         ("struct_size", C.c_uint32), ("precision", C.c_uint32), ("integrator", C.c_uint32),
         ("init_v", C.c_uint32), ("snapshot_every", C.c_uint32), ("accuracy", C.c_uint32),
+        ("rng", C.c_uint32), ("reserved", C.c_uint32),
         ("dt", C.c_double), ("gamma0", C.c_double), ("q", C.c_double), ("c", C.c_double),
         ("d", C.c_double), ("D", C.c_double), ("F0", C.c_double), ("A", C.c_double),
         ("omega", C.c_double), ("L", C.c_double), ("A1", C.c_double), ("A2", C.c_double),
@@ -91,7 +93,7 @@ def lib():
     return _lib
 
 
-_PARAM_KEYS = ["precision", "integrator", "init_v", "snapshot_every", "accuracy", "dt", "gamma0", "q", "c", "d",
+_PARAM_KEYS = ["precision", "integrator", "init_v", "snapshot_every", "accuracy", "rng", "dt", "gamma0", "q", "c", "d",
                "D", "F0", "A", "omega", "L", "A1", "A2", "phi", "v0", "e0", "traj_base",
                "traj_set_stride"]
 
@@ -216,7 +218,7 @@ class Ensemble:
     """
 
     def __init__(self, param_sets, n_particles, seed, snapshot_every=0, stream=None,
-                 traj_base=0, traj_set_stride=0, accuracy=ABM_ACCURACY_AUTO):
+                 traj_base=0, traj_set_stride=0, accuracy=ABM_ACCURACY_AUTO, rng=None):
         import torch
         self._torch = torch
         if not torch.cuda.is_available():
@@ -228,9 +230,11 @@ class Ensemble:
         if isinstance(param_sets, C.Array):      # already marshalled (make_params) by the caller
             params = param_sets
         else:
-            params = make_params(param_sets, stream=self.stream.cuda_stream,
-                                 snapshot_every=snapshot_every, traj_base=traj_base,
-                                 traj_set_stride=traj_set_stride, accuracy=accuracy)
+            common = dict(snapshot_every=snapshot_every, traj_base=traj_base,
+                          traj_set_stride=traj_set_stride, accuracy=accuracy)
+            if rng is not None:          # else the parameter records decide (default Philox)
+                common["rng"] = rng
+            params = make_params(param_sets, stream=self.stream.cuda_stream, **common)
         self.fp64 = int(params[0].precision) == 1
         self.ctx = abm_create(params, n_particles, self.n_sets, seed)
         self.frame = None

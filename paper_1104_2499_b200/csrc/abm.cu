@@ -34,7 +34,7 @@ struct abm_ctx {
   uint32_t magic;
   int device;
   cudaStream_t stream;
-  uint32_t precision, integrator, init_v, snap_every;
+  uint32_t precision, integrator, init_v, snap_every, rng;
   uint32_t n_sets;
   bool tilt;
   bool precise;         // fp32 accuracy mode resolved at create (include/abm.h, abm_params.accuracy)
@@ -43,6 +43,7 @@ struct abm_ctx {
   size_t real_size;
   void *x, *v, *e;      // state, SoA, Real[n_traj]
   void* xl;             // low part of x, float[n_traj] (precise fp32 mode only)
+  uint4* rng_state;     // xorshift state per trajectory (ABM_RNG_XORSHIFT128 only)
   void* coef_table;     // Coef<Real>[n_sets]
   void* tilt_table;     // Real[TILT_CHUNK + 1]
   double* partial;      // [n_sets * blocks_per_set][7]
@@ -129,13 +130,13 @@ int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets) {
   const abm_params& p0 = params[0];
   if (p0.struct_size != sizeof(abm_params)) return ABM_EINVAL;
   if (p0.precision > ABM_FP64 || p0.integrator > ABM_HEUN || p0.init_v > ABM_INIT_V_THERMAL ||
-      p0.accuracy > ABM_ACCURACY_PRECISE)
+      p0.accuracy > ABM_ACCURACY_PRECISE || p0.rng > ABM_RNG_XORSHIFT128)
     return ABM_EINVAL;
   for (uint32_t s = 0; s < n_sets; ++s) {
     const abm_params& p = params[s];
-    if (p.struct_size != sizeof(abm_params)) return ABM_EINVAL;
+    if (p.struct_size != sizeof(abm_params) || p.reserved != 0) return ABM_EINVAL;
     if (p.precision != p0.precision || p.integrator != p0.integrator || p.init_v != p0.init_v ||
-        p.accuracy != p0.accuracy || p.snapshot_every != p0.snapshot_every || p.dt != p0.dt || p.omega != p0.omega ||
+        p.accuracy != p0.accuracy || p.rng != p0.rng || p.snapshot_every != p0.snapshot_every || p.dt != p0.dt || p.omega != p0.omega ||
         p.traj_base != p0.traj_base || p.traj_set_stride != p0.traj_set_stride ||
         p.stream != p0.stream)
       return ABM_EINVAL;
@@ -194,7 +195,7 @@ void dev_free(abm_ctx* c, void* p) {
 }
 
 void free_all(abm_ctx* c) {
-  void* all[] = {c->x, c->v, c->e, c->xl, c->coef_table, c->tilt_table, c->partial, c->sums,
+  void* all[] = {c->x, c->v, c->e, c->xl, c->rng_state, c->coef_table, c->tilt_table, c->partial, c->sums,
                  c->moments, c->frame};
   for (void* p : all) dev_free(c, p);
   std::free(c->host_coefs);
@@ -243,27 +244,33 @@ int upload_coefs_and_init(abm_ctx* c, const abm_params* params) {
   init_kernel<Real><<<grid, 256, 0, c->stream>>>(
       static_cast<Real*>(c->x), static_cast<Real*>(c->v), static_cast<Real*>(c->e),
       static_cast<const Coef<Real>*>(c->coef_table), c->n_traj, c->n_particles, c->traj_base,
-      c->set_stride, c->seed, c->n_sets, c->init_v);
+      c->set_stride, c->seed, c->n_sets, c->init_v, c->rng_state);
   ABM_CK(c, cudaGetLastError());
   return ABM_OK;
 }
 
-template <typename Real, int INTEG, bool TILT, bool PRECISE>
+template <typename Real, int INTEG, bool TILT, bool PRECISE, bool XS>
 cudaError_t launch_step_p(const abm_ctx* c, const StepArgs<Real>& a) {
   const uint32_t grid = static_cast<uint32_t>((c->n_traj + STEP_BLOCK - 1) / STEP_BLOCK);
   if (c->n_sets == 1)
-    step_kernel<Real, INTEG, TILT, true, PRECISE><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+    step_kernel<Real, INTEG, TILT, true, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
   else
-    step_kernel<Real, INTEG, TILT, false, PRECISE><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+    step_kernel<Real, INTEG, TILT, false, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
   return cudaGetLastError();
+}
+
+template <typename Real, int INTEG, bool TILT, bool PRECISE>
+cudaError_t launch_step_r(const abm_ctx* c, const StepArgs<Real>& a) {
+  return c->rng == ABM_RNG_XORSHIFT128 ? launch_step_p<Real, INTEG, TILT, PRECISE, true>(c, a)
+                                       : launch_step_p<Real, INTEG, TILT, PRECISE, false>(c, a);
 }
 
 template <typename Real, int INTEG, bool TILT>
 cudaError_t launch_step_u(const abm_ctx* c, const StepArgs<Real>& a) {
   if constexpr (sizeof(Real) == 4) {  // the accuracy modes exist in fp32 only
-    if (c->precise) return launch_step_p<Real, INTEG, TILT, true>(c, a);
+    if (c->precise) return launch_step_r<Real, INTEG, TILT, true>(c, a);
   }
-  return launch_step_p<Real, INTEG, TILT, false>(c, a);
+  return launch_step_r<Real, INTEG, TILT, false>(c, a);
 }
 
 template <typename Real>
@@ -290,6 +297,7 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
   a.coef_table = static_cast<const Coef<Real>*>(c->coef_table);
   a.tilt = static_cast<const Real*>(c->tilt_table);
   a.snap = c->snap;
+  a.rng_state = c->rng_state;
   a.n_traj = c->n_traj;
   a.n_particles = c->n_particles;
   a.traj_base = c->traj_base;
@@ -382,6 +390,7 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   c->integrator = p0.integrator;
   c->init_v = p0.init_v;
   c->snap_every = p0.snapshot_every;
+  c->rng = p0.rng;
   c->n_sets = n_param_sets;
   c->n_particles = n_particles;
   c->n_traj = n_particles * n_param_sets;
@@ -436,6 +445,8 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   const size_t state_bytes = c->real_size * c->n_traj;
   if (!alloc(&c->x, state_bytes) || !alloc(&c->v, state_bytes) || !alloc(&c->e, state_bytes) ||
       (c->precise && !alloc(&c->xl, state_bytes)) ||
+      (c->rng == ABM_RNG_XORSHIFT128 &&
+       !alloc(reinterpret_cast<void**>(&c->rng_state), sizeof(uint4) * c->n_traj)) ||
       !alloc(reinterpret_cast<void**>(&c->partial),
              sizeof(double) * (N_SUMS - 1) * bps * n_param_sets) ||
       !alloc(reinterpret_cast<void**>(&c->sums), sizeof(double) * N_SUMS * n_param_sets) ||
@@ -637,6 +648,6 @@ const char* abm_strerror(int status) {
   }
 }
 
-uint32_t abm_abi_version(void) { return 3; }
+uint32_t abm_abi_version(void) { return 4; }
 
 }  // extern "C"

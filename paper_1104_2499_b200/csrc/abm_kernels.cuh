@@ -47,6 +47,7 @@ struct StepArgs {
   const Coef<Real>* coef_table;  // [n_sets] (used when !UNIFORM)
   const Real* tilt;              // tilt[j] = cos(omega (tilt_base + j) dt) (used when TILT)
   void* snap;                    // bound snapshot buffer or nullptr
+  uint4* rng_state;              // xorshift state per trajectory (used when XS), at a pair boundary
   uint64_t n_traj;               // local trajectories
   uint64_t n_particles;          // per set
   uint64_t traj_base, set_stride;
@@ -121,10 +122,12 @@ template <typename Real>
 __global__ void init_kernel(Real* __restrict__ x, Real* __restrict__ v, Real* __restrict__ e,
                             const Coef<Real>* __restrict__ coef_table, uint64_t n_traj,
                             uint64_t n_particles, uint64_t traj_base, uint64_t set_stride,
-                            uint64_t seed, uint32_t n_sets, uint32_t init_v) {
+                            uint64_t seed, uint32_t n_sets, uint32_t init_v,
+                            uint4* __restrict__ rng_state) {
   const uint64_t k = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (k >= n_traj) return;
   const TrajId id = traj_id(k, n_particles, traj_base, set_stride, n_sets == 1);
+  if (rng_state) rng_state[k] = xorshift_seed(seed, id.global);
   const Coef<Real> c = coef_table[id.set];
   const uint4 w = philox_block(seed, id.global, INIT_BLOCK);
   x[k] = init_x(c, w.x);
@@ -216,10 +219,14 @@ __device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf,
 // after the last one of a run is computed and dropped (its counter may wrap: harmless).
 constexpr int PHILOX_CHUNK = STEP_BLOCK;  // table entries per refill = threads per CTA
 
-template <typename Real, int INTEG, bool TILT, bool PRECISE, bool TABLE>
+//
+// XS (generator variant, NEXT-4): the words come from the trajectory's xorshift state S instead.
+// S always sits at a pair boundary -- before output 2 (n >> 1) -- when a step starts: whole blocks
+// draw four outputs; a single even step draws its pair from a copy, the odd step after it commits.
+template <typename Real, int INTEG, bool TILT, bool PRECISE, bool TABLE, bool XS>
 __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_t k, const bool active,
                                           const uint32_t traj_lo, const uint32_t traj_hi,
-                                          const Coef<Real>& cf, State<Real>& s) {
+                                          const Coef<Real>& cf, State<Real>& s, uint4& S) {
   __shared__ uint4 tab[TABLE ? 2 : 1][TABLE ? PHILOX_CHUNK : 1];
   uint32_t par = 0;
   const uint32_t k0 = static_cast<uint32_t>(a.seed), k1 = static_cast<uint32_t>(a.seed >> 32);
@@ -247,6 +254,32 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
       const Real* tl = TILT ? a.tilt + (n - a.tilt_base) : nullptr;
       uint64_t to_snap = (K && snap_aligned) ? (next_snap - n) >> 2 : ~0ull;  // blocks to the frame
       uint32_t left = nb;
+      if (XS) {
+        // The look-ahead block is drawn for every block but the last of the run, so that exactly
+        // 4 nb outputs are consumed.
+        uint4 w = xorshift128_x4(S);
+        do {
+          const uint32_t seg = left < to_snap ? left : static_cast<uint32_t>(to_snap);  // >= 1
+          const bool last = seg == left;
+          uint32_t ahead = last ? seg - 1u : seg;  // blocks of this segment with a look-ahead draw
+#pragma unroll 1
+          for (; ahead; --ahead) {
+            const uint4 w_next = xorshift128_x4(S);
+            four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+            w = w_next;
+          }
+          if (last) four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+          left -= seg;
+          if (seg == to_snap) {  // a frame is due after this block
+            if (active) store_snapshot(a.snap, a.snap_stride, k, s);
+            to_snap = K >> 2;
+          } else {
+            to_snap -= seg;
+          }
+        } while (left);
+        n += static_cast<uint64_t>(nb) << 2;
+        if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
+      } else {
       uint4 w = philox4x32_10(b_lo, b_hi, traj_lo, traj_hi, k0, k1);
       if (TABLE) {
         const PhiloxTraj pt = philox_traj(traj_lo, b_hi, k0);
@@ -304,9 +337,20 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
       }
       n += static_cast<uint64_t>(nb) << 2;
       if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
+      }
     } else {
       // ---- slow path: one step (unaligned head / tail, or K not a multiple of 4) ----
-      const uint4 w = philox_block(a.seed, (static_cast<uint64_t>(traj_hi) << 32) | traj_lo, n >> 2);
+      uint4 w;
+      if (XS) {
+        // the pair of steps (n & ~1, n | 1) from a copy of S; the odd step commits the advance.
+        // The pair is placed where the Philox code below expects the pair of step n.
+        uint4 T = S;
+        const uint32_t wa = xorshift128(T), wb = xorshift128(T);
+        w = make_uint4(wa, wb, wa, wb);
+        if (n & 1u) S = T;
+      } else {
+        w = philox_block(a.seed, (static_cast<uint64_t>(traj_hi) << 32) | traj_lo, n >> 2);
+      }
       const Noise4<Real> z(w, cf);
       const bool second = (n >> 1) & 1u;
       const Real rho = Noise4<Real>::SIGN * (second ? z.b.rho : z.a.rho);
@@ -330,7 +374,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
 #define ABM_PHILOX_TABLE 1
 #endif
 
-template <typename Real, int INTEG, bool TILT, bool UNIFORM, bool PRECISE>
+template <typename Real, int INTEG, bool TILT, bool UNIFORM, bool PRECISE, bool XS>
 __global__ void __launch_bounds__(STEP_BLOCK, step_min_blocks<Real, INTEG, UNIFORM>())
 step_kernel(const __grid_constant__ StepArgs<Real> a) {
   const uint64_t k_raw = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
@@ -356,18 +400,25 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
   // High word of the global trajectory index (Philox counter word 3): the host passes it as a
   // kernel parameter when the whole launch shares one value (always, unless the index range
   // straddles a multiple of 2^32); the block-head table of run_steps needs that.
-  if (a.traj_hi_shared)
-    run_steps<Real, INTEG, TILT, PRECISE, ABM_PHILOX_TABLE != 0>(
-        a, k, active, static_cast<uint32_t>(id.global), a.traj_hi, cf, s);
-  else
-    run_steps<Real, INTEG, TILT, PRECISE, false>(a, k, active, static_cast<uint32_t>(id.global),
-                                                 static_cast<uint32_t>(id.global >> 32), cf, s);
+  uint4 S = make_uint4(0u, 0u, 0u, 0u);
+  if (XS) {
+    S = a.rng_state[k];
+    run_steps<Real, INTEG, TILT, PRECISE, false, true>(a, k, active, 0u, 0u, cf, s, S);
+  } else if (a.traj_hi_shared) {
+    run_steps<Real, INTEG, TILT, PRECISE, ABM_PHILOX_TABLE != 0, false>(
+        a, k, active, static_cast<uint32_t>(id.global), a.traj_hi, cf, s, S);
+  } else {
+    run_steps<Real, INTEG, TILT, PRECISE, false, false>(
+        a, k, active, static_cast<uint32_t>(id.global), static_cast<uint32_t>(id.global >> 32), cf,
+        s, S);
+  }
 
   if (active) {
     a.x[k] = s.x;
     a.v[k] = s.v;
     a.e[k] = s.e;
     if (PRECISE) a.xl[k] = s.xl;
+    if (XS) a.rng_state[k] = S;
   }
 }
 

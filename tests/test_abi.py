@@ -34,7 +34,7 @@ def test_every_declared_symbol_is_exported(abm):
     L = abm.lib()
     for n in names:
         assert getattr(L, n) is not None
-    assert L.abm_abi_version() == 3
+    assert L.abm_abi_version() == 4
 
 
 def test_header_is_plain_c_and_layout_matches_ctypes(abm, tmp_path):

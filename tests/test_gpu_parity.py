@@ -449,3 +449,71 @@ def test_paper_f0_sweep_time_averaged_velocity(abm, oracle):
         assert scale_rel_err(st[s], np.stack([x, v, e], 1)).max() <= 1e-4   # 400 steps of error growth
     # a strong load drags the particle its way (reading G13: +F0 as printed)
     assert vbar[0] < -0.2 and vbar[-1] > 0.2
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4  generator variant: per-trajectory xorshift128 state
+# ---------------------------------------------------------------------------------------------
+
+def test_xorshift_normals_consumed_by_the_step_kernel(abm, oracle):
+    """Same construction as for Philox: v_{n+1} = sigma z_n = z_n, one launch per step, so odd launches
+    start in the middle of a pair and must re-draw it from the stored state."""
+    dt = 2.0**-10
+    p = dict(W.DEFAULTS, rng=1, A1=0.0, A2=0.0, d=0.0, q=0.0, c=0.0, gamma0=1.0 / dt, dt=dt, D=0.5 / dt)
+    N, seed = 1500, 424242
+    want = np.array([[oracle.normal_xorshift(seed, k, n, 0) for n in range(10)] for k in range(0, N, 50)])
+    with abm.Ensemble([p], N, seed) as ens:
+        for n in range(10):
+            ens.step(1)
+            z = ens.state()[::50, 1]
+            rho = np.hypot(want[:, n & ~1], want[:, n | 1])
+            bound = 1.7e-7 / np.maximum(rho, 1e-4) + 1.0e-6 * (1.0 + rho)
+            assert np.all(np.abs(z - want[:, n]) <= bound), n
+
+
+XS_CASES = [
+    ("cfg0", W.config0, 1000, None, TOL_F32),
+    ("cfg2", W.config2, 64, 12, TOL_F32),
+    ("cfg3", W.config3, 777, None, TOL_F32),
+    ("cfg4", W.config4, 513, None, TOL_F64),
+]
+
+
+@pytest.mark.parametrize("name,mk,n_particles,n_sets,tol", XS_CASES, ids=[c[0] for c in XS_CASES])
+def test_xorshift_state_after_100_steps(abm, oracle, name, mk, n_particles, n_sets, tol):
+    wl = mk()
+    sets = [dict(p, rng=1) for p in small(wl, n_particles, n_sets if wl.n_param_sets > 1 else None)]
+    with abm.Ensemble(sets, n_particles, wl.seed) as ens:
+        ens.step(100)
+        got = ens.state().reshape(len(sets), n_particles, 3)
+    for s, p in enumerate(sets):
+        first = s * n_particles
+        x, v, e = oracle.init_many(p, wl.seed, n_particles, first)
+        oracle.run(p, wl.seed, x, v, e, 0, 100, first)
+        err = scale_rel_err(got[s], np.stack([x, v, e], 1))
+        assert np.all(err <= tol), (name, s, err)
+
+
+@pytest.mark.parametrize("mk,n,K", [(W.config0, 300, 0), (W.config0, 300, 6), (W.config0, 259, 8),
+                                    (W.config3, 200, 0), (W.config4, 129, 0)])
+def test_xorshift_split_launches_are_bit_identical(abm, torch, mk, n, K):
+    wl = mk()
+    p = dict(wl.set_params(0), rng=1)
+    with abm.Ensemble([p], n, wl.seed, snapshot_every=K) as a, abm.Ensemble([p], n, wl.seed, snapshot_every=K) as b:
+        fa = a.bind_snapshot() if K else None
+        fb = b.bind_snapshot() if K else None
+        a.step(61)
+        for part in (1, 2, 3, 5, 4, 7, 8, 13, 18):        # 61 steps through odd and even boundaries
+            b.step(part)
+        sa, sb = a.state(), b.state()
+        assert np.array_equal(sa, sb)
+        if K:
+            torch.cuda.synchronize()
+            assert torch.equal(fa, fb)
+        a.step(11)
+        b.step(11)
+        assert np.array_equal(a.state(), b.state())
+    # and the Philox stream gives something else from the same seed
+    with abm.Ensemble([dict(p, rng=0)], n, wl.seed) as c:
+        c.step(72)
+        assert not np.array_equal(c.state(), sa)
