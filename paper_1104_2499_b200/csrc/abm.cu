@@ -42,7 +42,7 @@ struct abm_ctx {
   double dt, omega;
   size_t real_size;
   void *x, *v, *e;      // state, SoA, Real[n_traj]
-  void* xl;             // low part of x, float[n_traj] (precise fp32 mode only)
+  void* xl;             // high word of the fixed-point position, [n_traj] (precise fp32 mode only)
   uint4* rng_state;     // xorshift state per trajectory (ABM_RNG_XORSHIFT128 only)
   void* coef_table;     // Coef<Real>[n_sets]
   void* tilt_table;     // Real[TILT_CHUNK + 1]
@@ -97,7 +97,8 @@ Coef<Real> make_coef(const abm_params& p) {
     c.s2 = static_cast<Real>(std::sqrt(2.0 * p.D * p.dt));  // sigma
   }
   c.bm_o = static_cast<Real>(two_pi * 0x1p-24 - 1.5 * two_pi);
-  c.inv_L = static_cast<Real>(1.0 / p.L);
+  c.dtS = static_cast<Real>(p.dt * 4294967296.0 / p.L);
+  c.hdtS = static_cast<Real>(0.5 * p.dt * 4294967296.0 / p.L);
   c.A = static_cast<Real>(p.A);
   c.L = static_cast<Real>(p.L);
   c.v0 = static_cast<Real>(p.v0);
@@ -244,7 +245,7 @@ int upload_coefs_and_init(abm_ctx* c, const abm_params* params) {
   init_kernel<Real><<<grid, 256, 0, c->stream>>>(
       static_cast<Real*>(c->x), static_cast<Real*>(c->v), static_cast<Real*>(c->e),
       static_cast<const Coef<Real>*>(c->coef_table), c->n_traj, c->n_particles, c->traj_base,
-      c->set_stride, c->seed, c->n_sets, c->init_v, c->rng_state);
+      c->set_stride, c->seed, c->n_sets, c->init_v, c->rng_state, static_cast<Real*>(c->xl));
   ABM_CK(c, cudaGetLastError());
   return ABM_OK;
 }
@@ -334,7 +335,8 @@ int reduce_moments(abm_ctx* c) {
   const uint32_t grid = c->n_sets * c->blocks_per_set;
   moments_partial_kernel<Real><<<grid, c->mom_block, 0, c->stream>>>(
       static_cast<const Real*>(c->x), static_cast<const Real*>(c->v),
-      static_cast<const Real*>(c->e), static_cast<const Coef<Real>*>(c->coef_table),
+      static_cast<const Real*>(c->e), static_cast<const Real*>(c->xl),
+      static_cast<const Coef<Real>*>(c->coef_table),
       c->n_particles, c->traj_base, c->set_stride, c->seed, c->blocks_per_set, c->mom_slice,
       c->partial);
   ABM_CK(c, cudaGetLastError());
@@ -359,11 +361,14 @@ int write_frame(abm_ctx* c, void* dev_ptr, uint32_t stride) {
   if (c->precision == ABM_FP32)
     snapshot_kernel<float><<<grid, 256, 0, c->stream>>>(
         static_cast<const float*>(c->x), static_cast<const float*>(c->v),
-        static_cast<const float*>(c->e), c->n_traj, dev_ptr, stride);
+        static_cast<const float*>(c->e), static_cast<const float*>(c->xl),
+        static_cast<const Coef<float>*>(c->coef_table), c->n_traj, c->n_particles, c->n_sets, dev_ptr,
+        stride);
   else
     snapshot_kernel<double><<<grid, 256, 0, c->stream>>>(
         static_cast<const double*>(c->x), static_cast<const double*>(c->v),
-        static_cast<const double*>(c->e), c->n_traj, dev_ptr, stride);
+        static_cast<const double*>(c->e), nullptr, static_cast<const Coef<double>*>(c->coef_table),
+        c->n_traj, c->n_particles, c->n_sets, dev_ptr, stride);
   ABM_CK(c, cudaGetLastError());
   return ABM_OK;
 }
@@ -453,8 +458,6 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
       !alloc(reinterpret_cast<void**>(&c->moments), sizeof(MomentRec) * n_param_sets) ||
       (c->tilt && !alloc(&c->tilt_table, c->real_size * (TILT_CHUNK + 1))))
     return fail(rc);
-  if (c->precise && cudaMemsetAsync(c->xl, 0, state_bytes, c->stream) != cudaSuccess)
-    return fail(ABM_ECUDA);
   rc = c->precision == ABM_FP32 ? upload_coefs_and_init<float>(c, params)
                                 : upload_coefs_and_init<double>(c, params);
   if (rc != ABM_OK) return fail(rc);
@@ -554,13 +557,14 @@ int abm_raster(abm_ctx* c, uint32_t* dev_counts, uint32_t width, uint32_t height
     using Real = decltype(real_tag);
     const Real* x = static_cast<const Real*>(c->x);
     const Real* v = static_cast<const Real*>(c->v);
+    const Real* xl = static_cast<const Real*>(c->xl);
     const Coef<Real>* tab = static_cast<const Coef<Real>*>(c->coef_table);
     if (smem)
       raster_kernel<Real, true><<<grid, RASTER_BLOCK, sizeof(uint32_t) * n_bins, c->stream>>>(
-          x, v, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range, dev_counts);
+          x, v, xl, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range, dev_counts);
     else
       raster_kernel<Real, false><<<grid, RASTER_BLOCK, 0, c->stream>>>(
-          x, v, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range, dev_counts);
+          x, v, xl, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range, dev_counts);
   };
   if (c->precision == ABM_FP32) launch(float{}); else launch(double{});
   ABM_CK(c, cudaGetLastError());

@@ -43,7 +43,7 @@ struct StepArgs {
   Real* x;
   Real* v;
   Real* e;
-  Real* xl;                      // low part of x (used when PRECISE; else nullptr)
+  Real* xl;                      // high word of the fixed-point position (PRECISE; else nullptr)
   const Coef<Real>* coef_table;  // [n_sets] (used when !UNIFORM)
   const Real* tilt;              // tilt[j] = cos(omega (tilt_base + j) dt) (used when TILT)
   void* snap;                    // bound snapshot buffer or nullptr
@@ -107,30 +107,42 @@ __device__ __forceinline__ void store_snapshot(void* snap, uint32_t stride, uint
 
 template <typename Real>
 __global__ void snapshot_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
-                                const Real* __restrict__ e, uint64_t n_traj, void* snap,
-                                uint32_t stride) {
+                                const Real* __restrict__ e, const Real* __restrict__ xl,
+                                const Coef<Real>* __restrict__ coef_table, uint64_t n_traj,
+                                uint64_t n_particles, uint32_t n_sets, void* snap, uint32_t stride) {
   const uint64_t k = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (k >= n_traj) return;
-  State<Real> s{x[k], v[k], e[k], Real(0)};
+  const uint32_t set = n_sets == 1 ? 0u : static_cast<uint32_t>(k / n_particles);
+  State<Real> s{load_position(x, xl, k, coef_table[set].L), v[k], e[k], Real(0), 0u, 0};
   store_snapshot(snap, stride, k, s);
 }
 
 // ---------------------------------------------------------------------------------------------
 // S0  init
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void store_fixed(float* x, float* xl, uint64_t k, uint32_t xf, int32_t xc) {
+  x[k] = __uint_as_float(xf);
+  xl[k] = __int_as_float(xc);
+}
+__device__ __forceinline__ void store_fixed(double*, double*, uint64_t, uint32_t, int32_t) {}
+
 template <typename Real>
 __global__ void init_kernel(Real* __restrict__ x, Real* __restrict__ v, Real* __restrict__ e,
                             const Coef<Real>* __restrict__ coef_table, uint64_t n_traj,
                             uint64_t n_particles, uint64_t traj_base, uint64_t set_stride,
                             uint64_t seed, uint32_t n_sets, uint32_t init_v,
-                            uint4* __restrict__ rng_state) {
+                            uint4* __restrict__ rng_state, Real* __restrict__ xl) {
   const uint64_t k = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (k >= n_traj) return;
   const TrajId id = traj_id(k, n_particles, traj_base, set_stride, n_sets == 1);
   if (rng_state) rng_state[k] = xorshift_seed(seed, id.global);
   const Coef<Real> c = coef_table[id.set];
   const uint4 w = philox_block(seed, id.global, INIT_BLOCK);
-  x[k] = init_x(c, w.x);
+  if (xl) {  // precise fp32 mode: X = x0 2^32 / L = (w0 >> 8) << 8 exactly; the arrays hold its words
+    store_fixed(x, xl, k, w.x & 0xffffff00u, 0);
+  } else {
+    x[k] = init_x(c, w.x);
+  }
   v[k] = init_v ? init_v_thermal(c, w.z, w.w) : c.v0;
   e[k] = c.e0;
 }
@@ -198,6 +210,14 @@ __device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf,
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.sn, t1, t2);
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.cs, t2, t3);
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.sn, t3, t4);
+}
+
+// The state as a frame shows it: in precise mode x is the remainder, the frame wants the position.
+template <bool PRECISE, typename Real>
+__device__ __forceinline__ State<Real> frame_state(const State<Real>& s, const Coef<Real>& cf) {
+  State<Real> o = s;
+  if constexpr (PRECISE) o.x = position_fixed(s.xf, s.xc, cf.L);
+  return o;
 }
 
 // The step loop of one trajectory.
@@ -271,7 +291,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
           if (last) four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
           left -= seg;
           if (seg == to_snap) {  // a frame is due after this block
-            if (active) store_snapshot(a.snap, a.snap_stride, k, s);
+            if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
             to_snap = K >> 2;
           } else {
             to_snap -= seg;
@@ -306,7 +326,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
             } while (++tp != tp_end);
             done += seg;
             if (seg == to_snap) {  // a frame is due after this block
-              if (active) store_snapshot(a.snap, a.snap_stride, k, s);
+              if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
               to_snap = K >> 2;
             } else {
               to_snap -= seg;
@@ -328,7 +348,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
           } while (++b_lo != seg_end);
           left -= seg;
           if (seg == to_snap) {  // a frame is due after this block
-            if (active) store_snapshot(a.snap, a.snap_stride, k, s);
+            if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
             to_snap = K >> 2;
           } else {
             to_snap -= seg;
@@ -364,7 +384,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
       ++n;
     }
     if (n == next_snap) {
-      if (active) store_snapshot(a.snap, a.snap_stride, k, s);
+      if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
       next_snap += K;
     }
   }
@@ -395,7 +415,11 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
     cf.bm_o = g->bm_o;
   }
 
-  State<Real> s{a.x[k], a.v[k], a.e[k], PRECISE ? a.xl[k] : Real(0)};
+  State<Real> s{a.x[k], a.v[k], a.e[k], Real(0), 0u, 0};
+  if constexpr (PRECISE) {  // the arrays hold the two words of the fixed-point position
+    s.xf = __float_as_uint(a.x[k]);
+    s.xc = __float_as_int(a.xl[k]);
+  }
 
   // High word of the global trajectory index (Philox counter word 3): the host passes it as a
   // kernel parameter when the whole launch shares one value (always, unless the index range
@@ -414,10 +438,10 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
   }
 
   if (active) {
-    a.x[k] = s.x;
+    if constexpr (PRECISE) store_fixed(a.x, a.xl, k, s.xf, s.xc);
+    else a.x[k] = s.x;
     a.v[k] = s.v;
     a.e[k] = s.e;
-    if (PRECISE) a.xl[k] = s.xl;
     if (XS) a.rng_state[k] = S;
   }
 }
@@ -431,7 +455,8 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
 template <typename Real>
 __global__ void __launch_bounds__(MOM_BLOCK)
 moments_partial_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
-                       const Real* __restrict__ e, const Coef<Real>* __restrict__ coef_table,
+                       const Real* __restrict__ e, const Real* __restrict__ xl,
+                       const Coef<Real>* __restrict__ coef_table,
                        uint64_t n_particles, uint64_t traj_base, uint64_t set_stride, uint64_t seed,
                        uint32_t blocks_per_set, uint32_t slice, double* __restrict__ partial) {
   const uint32_t set = blockIdx.x / blocks_per_set;
@@ -445,7 +470,7 @@ moments_partial_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
     const uint64_t k = static_cast<uint64_t>(set) * n_particles + r;
     const uint64_t g = traj_base + static_cast<uint64_t>(set) * set_stride + r;
     const uint4 w = philox_block(seed, g, INIT_BLOCK);
-    const double xi = static_cast<double>(x[k]);
+    const double xi = static_cast<double>(load_position(x, xl, k, c.L));
     const double vi = static_cast<double>(v[k]);
     const double dx = xi - static_cast<double>(init_x(c, w.x));
     acc[0] += xi;
@@ -560,7 +585,7 @@ __device__ __forceinline__ uint32_t raster_bin(double x, double v, double L, dou
 
 template <typename Real, bool SMEM>
 __global__ void __launch_bounds__(RASTER_BLOCK)
-raster_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
+raster_kernel(const Real* __restrict__ x, const Real* __restrict__ v, const Real* __restrict__ xl,
               const Coef<Real>* __restrict__ coef_table, uint64_t n_traj, uint64_t n_particles,
               uint32_t n_sets, uint32_t W, uint32_t H, double v_min, double v_range,
               uint32_t* __restrict__ counts) {
@@ -574,8 +599,10 @@ raster_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
   for (uint64_t k = static_cast<uint64_t>(blockIdx.x) * RASTER_BLOCK + threadIdx.x; k < n_traj;
        k += stride) {
     const uint32_t set = n_sets == 1 ? 0u : static_cast<uint32_t>(k / n_particles);
-    const double L = static_cast<double>(coef_table[set].L);
-    const uint32_t bin = raster_bin(static_cast<double>(x[k]), static_cast<double>(v[k]), L, v_min,
+    const Real Lr = coef_table[set].L;
+    const double L = static_cast<double>(Lr);
+    const uint32_t bin = raster_bin(static_cast<double>(load_position(x, xl, k, Lr)),
+                                    static_cast<double>(v[k]), L, v_min,
                                     v_range, W, H);
     if (bin != 0xffffffffu) {
       if (SMEM) atomicAdd(&hist[bin], 1u);
