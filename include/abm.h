@@ -65,11 +65,12 @@ enum { ABM_INIT_V_CONST = 0, ABM_INIT_V_THERMAL = 1 }; /* abm_params.init_v */
 /* abm_params.accuracy -- "precise vs fast intrinsics chosen against the stated tolerance"
  * (BASELINE.json north_star (b): fp32 state within 1e-5 of the fp64 oracle after 100 steps).
  *   FAST     angle 2 pi (x + phi) / L handed to MUFU.COS as is; x' = x + dt v in one FMA.
- *   PRECISE  the state carries the position as (whole periods, remainder): the remainder stays
- *            within about half a period of 0, so the angle and the x update are rounded at that
- *            magnitude instead of the unwrapped position's; renormalised every fourth step:
- *            +1 FP32 instruction per step, one more float of state per trajectory.  Frames, moments
- *            and the raster see the position periods * L + remainder rounded once to fp32.
+ *   PRECISE  the state carries the position as a 64-bit fixed-point number of periods (changed by
+ *            exact integer additions only) plus a float offset that collects the increments of at
+ *            most four steps, so nothing is rounded at the magnitude of the unwrapped position;
+ *            the force takes its angle from the fraction word.  About +1.5 instructions per step
+ *            over FAST, two more words of state per trajectory.  Frames, moments and the raster see
+ *            the position rounded once to fp32.  Needs 4 |v| dt < L / 2.
  *   AUTO     PRECISE if dt (2 pi / L)^2 (|A1| + 4 |A2|) > 0.15 for any set, else FAST
  *            (configs[0-2]: 0.079 -> FAST; config[3]: 0.39 -> PRECISE).
  * Ignored in fp64.  Both modes consume the same random stream. */

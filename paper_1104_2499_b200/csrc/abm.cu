@@ -42,7 +42,8 @@ struct abm_ctx {
   double dt, omega;
   size_t real_size;
   void *x, *v, *e;      // state, SoA, Real[n_traj]
-  void* xl;             // high word of the fixed-point position, [n_traj] (precise fp32 mode only)
+  void* xl;             // precise fp32 mode only: fraction word of the fixed-point position, [n_traj]
+  void* xh;             //   and its whole periods (the x array then holds the float offset)
   uint4* rng_state;     // xorshift state per trajectory (ABM_RNG_XORSHIFT128 only)
   void* coef_table;     // Coef<Real>[n_sets]
   void* tilt_table;     // Real[TILT_CHUNK + 1]
@@ -97,8 +98,7 @@ Coef<Real> make_coef(const abm_params& p) {
     c.s2 = static_cast<Real>(std::sqrt(2.0 * p.D * p.dt));  // sigma
   }
   c.bm_o = static_cast<Real>(two_pi * 0x1p-24 - 1.5 * two_pi);
-  c.dtS = static_cast<Real>(p.dt * 4294967296.0 / p.L);
-  c.hdtS = static_cast<Real>(0.5 * p.dt * 4294967296.0 / p.L);
+  c.fxS = static_cast<Real>(4294967296.0 / p.L);
   c.A = static_cast<Real>(p.A);
   c.L = static_cast<Real>(p.L);
   c.v0 = static_cast<Real>(p.v0);
@@ -196,7 +196,7 @@ void dev_free(abm_ctx* c, void* p) {
 }
 
 void free_all(abm_ctx* c) {
-  void* all[] = {c->x, c->v, c->e, c->xl, c->rng_state, c->coef_table, c->tilt_table, c->partial, c->sums,
+  void* all[] = {c->x, c->v, c->e, c->xl, c->xh, c->rng_state, c->coef_table, c->tilt_table, c->partial, c->sums,
                  c->moments, c->frame};
   for (void* p : all) dev_free(c, p);
   std::free(c->host_coefs);
@@ -245,7 +245,8 @@ int upload_coefs_and_init(abm_ctx* c, const abm_params* params) {
   init_kernel<Real><<<grid, 256, 0, c->stream>>>(
       static_cast<Real*>(c->x), static_cast<Real*>(c->v), static_cast<Real*>(c->e),
       static_cast<const Coef<Real>*>(c->coef_table), c->n_traj, c->n_particles, c->traj_base,
-      c->set_stride, c->seed, c->n_sets, c->init_v, c->rng_state, static_cast<Real*>(c->xl));
+      c->set_stride, c->seed, c->n_sets, c->init_v, c->rng_state, static_cast<Real*>(c->xl),
+      static_cast<Real*>(c->xh));
   ABM_CK(c, cudaGetLastError());
   return ABM_OK;
 }
@@ -295,6 +296,7 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
   a.v = static_cast<Real*>(c->v);
   a.e = static_cast<Real*>(c->e);
   a.xl = static_cast<Real*>(c->xl);
+  a.xh = static_cast<Real*>(c->xh);
   a.coef_table = static_cast<const Coef<Real>*>(c->coef_table);
   a.tilt = static_cast<const Real*>(c->tilt_table);
   a.snap = c->snap;
@@ -336,7 +338,7 @@ int reduce_moments(abm_ctx* c) {
   moments_partial_kernel<Real><<<grid, c->mom_block, 0, c->stream>>>(
       static_cast<const Real*>(c->x), static_cast<const Real*>(c->v),
       static_cast<const Real*>(c->e), static_cast<const Real*>(c->xl),
-      static_cast<const Coef<Real>*>(c->coef_table),
+      static_cast<const Real*>(c->xh), static_cast<const Coef<Real>*>(c->coef_table),
       c->n_particles, c->traj_base, c->set_stride, c->seed, c->blocks_per_set, c->mom_slice,
       c->partial);
   ABM_CK(c, cudaGetLastError());
@@ -362,12 +364,13 @@ int write_frame(abm_ctx* c, void* dev_ptr, uint32_t stride) {
     snapshot_kernel<float><<<grid, 256, 0, c->stream>>>(
         static_cast<const float*>(c->x), static_cast<const float*>(c->v),
         static_cast<const float*>(c->e), static_cast<const float*>(c->xl),
-        static_cast<const Coef<float>*>(c->coef_table), c->n_traj, c->n_particles, c->n_sets, dev_ptr,
+        static_cast<const float*>(c->xh), static_cast<const Coef<float>*>(c->coef_table), c->n_traj, c->n_particles, c->n_sets, dev_ptr,
         stride);
   else
     snapshot_kernel<double><<<grid, 256, 0, c->stream>>>(
         static_cast<const double*>(c->x), static_cast<const double*>(c->v),
-        static_cast<const double*>(c->e), nullptr, static_cast<const Coef<double>*>(c->coef_table),
+        static_cast<const double*>(c->e), nullptr, nullptr,
+        static_cast<const Coef<double>*>(c->coef_table),
         c->n_traj, c->n_particles, c->n_sets, dev_ptr, stride);
   ABM_CK(c, cudaGetLastError());
   return ABM_OK;
@@ -449,7 +452,7 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   };
   const size_t state_bytes = c->real_size * c->n_traj;
   if (!alloc(&c->x, state_bytes) || !alloc(&c->v, state_bytes) || !alloc(&c->e, state_bytes) ||
-      (c->precise && !alloc(&c->xl, state_bytes)) ||
+      (c->precise && (!alloc(&c->xl, state_bytes) || !alloc(&c->xh, state_bytes))) ||
       (c->rng == ABM_RNG_XORSHIFT128 &&
        !alloc(reinterpret_cast<void**>(&c->rng_state), sizeof(uint4) * c->n_traj)) ||
       !alloc(reinterpret_cast<void**>(&c->partial),
@@ -558,13 +561,16 @@ int abm_raster(abm_ctx* c, uint32_t* dev_counts, uint32_t width, uint32_t height
     const Real* x = static_cast<const Real*>(c->x);
     const Real* v = static_cast<const Real*>(c->v);
     const Real* xl = static_cast<const Real*>(c->xl);
+    const Real* xh = static_cast<const Real*>(c->xh);
     const Coef<Real>* tab = static_cast<const Coef<Real>*>(c->coef_table);
     if (smem)
       raster_kernel<Real, true><<<grid, RASTER_BLOCK, sizeof(uint32_t) * n_bins, c->stream>>>(
-          x, v, xl, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range, dev_counts);
+          x, v, xl, xh, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range,
+          dev_counts);
     else
       raster_kernel<Real, false><<<grid, RASTER_BLOCK, 0, c->stream>>>(
-          x, v, xl, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range, dev_counts);
+          x, v, xl, xh, tab, c->n_traj, c->n_particles, c->n_sets, width, height, v_min, v_range,
+          dev_counts);
   };
   if (c->precision == ABM_FP32) launch(float{}); else launch(double{});
   ABM_CK(c, cudaGetLastError());

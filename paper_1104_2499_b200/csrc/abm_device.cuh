@@ -182,7 +182,8 @@ struct Coef {
   Real A;              // tilt amplitude
   Real L, v0, e0, sv;  // init: x0 = L u, v0, e0, sv = sqrt(D/gamma0)
   Real bm_o;           // fp32: 2 pi 2^-24 - 3 pi, offset of the Box-Muller angle (see S2)
-  Real dtS, hdtS;      // precise fp32 mode: dt 2^32 / L and half of it (fixed-point position, S4)
+  Real fxS;            // precise fp32 mode: 2^32 / L, length -> fixed-point units (S4)
+  Real pad;
 };
 static_assert(sizeof(Coef<float>) == 80, "Coef<float> layout");
 static_assert(sizeof(Coef<double>) == 160, "Coef<double> layout");
@@ -190,9 +191,11 @@ static_assert(sizeof(Coef<double>) == 160, "Coef<double> layout");
 template <typename Real>
 struct State {
   Real x, v, e;
-  Real xl;       // unused in registers (the xl ARRAY holds xc in precise fp32 mode)
-  uint32_t xf;   // precise fp32 mode only: the position as 32.32 fixed point in units of L,
-  int32_t xc;    //   X = xc * 2^32 + xf = x 2^32 / L  (x, xl unused then)
+  Real xl;       // unused
+  // precise fp32 mode only (see "Precise fp32 mode" below): the position is (xc 2^32 + xf) L 2^-32 + x
+  uint32_t xf;   //   fraction of a period, 32-bit fixed point
+  int32_t xc;    //   whole periods
+  Real thb;      //   angle of the fixed-point part, 2 pi xf 2^-32 + phase (recomputed, not stored)
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -351,16 +354,16 @@ __device__ __forceinline__ Normal2d box_muller_f64(uint32_t wa, uint32_t wb, dou
 // cos 2th = 2 cos^2 th - 1  (Eq. 3).
 //
 // fp32: th = th_s x + th_o in radians goes to MUFU.COS through the range-scale multiply ptxas puts
-// in front of it: two roundings at the magnitude of th, up to ~2.4e-6 rad for |x| ~ 3 L (fast
-// mode; precise mode uses force_fixed below).
+// in front of it: two roundings at the magnitude of th, up to ~2.4e-6 rad for |x| ~ 3 L in fast
+// mode; in precise mode x is a small offset and thb the angle of the fixed-point part (S4).
 // ---------------------------------------------------------------------------------------------
 template <bool PRECISE>
-__device__ __forceinline__ float force(const Coef<float>& k, float x, float k0t) {
-  const float c = fast_cos(__fmaf_rn(x, k.th_s, k.th_o));
+__device__ __forceinline__ float force(const Coef<float>& k, float x, float k0t, float thb) {
+  const float c = fast_cos(__fmaf_rn(x, k.th_s, PRECISE ? thb : k.th_o));
   return __fmaf_rn(__fmaf_rn(k.k2, c, k.k1), c, k0t);
 }
 template <bool PRECISE>
-__device__ __forceinline__ double force(const Coef<double>& k, double x, double k0t) {
+__device__ __forceinline__ double force(const Coef<double>& k, double x, double k0t, double) {
   const double c = cospi_f64(__fma_rn(x, k.th_s, k.th_o));
   return __fma_rn(__fma_rn(k.k2, c, k.k1), c, k0t);
 }
@@ -386,56 +389,56 @@ __device__ __forceinline__ double add_(double a, double b) { return __dadd_rn(a,
 // Precise fp32 mode: what limits the 100-step agreement with the fp64
 // oracle is rounding at the magnitude of the unwrapped position -- of the angle 2 pi (x + phi) / L
 // and of x' = x + dt v (the error random-walks and is amplified each step by dt U'').  Here the
-// position is a 64-bit fixed-point number X = x 2^32 / L (high word xc = whole periods, low word
-// xf = fraction of a period, resolution 2.3e-10 L):
-//   * the increment is rounded once to an integer, rni(v dt 2^32 / L) (F2I, a conversion-pipe
-//     instruction) and ADDED EXACTLY (IADD3 + IADD3.X on the ALU pipe) -- no rounding at the
-//     magnitude of x at all, no compensation terms;
-//   * the force needs x mod L only: the signed low word, converted to float (I2F: relative
-//     2^-25 of at most half a period), is the angle in units of 2 pi 2^-32 rad -- no period
-//     removal; the predictor of Heun's scheme adds its angle increment to that angle.
-// Per step this takes FP32 work OFF the FMA dispatch port (the loop's binding resource): the x
-// update becomes FMUL + F2I + two integer adds.  Valid while |v dt| < L / 2 per step (F2I
-// saturates beyond; such a step size resolves nothing of the potential anyway).
+// position is split as  X L 2^-32 + x:
+//   * X = xc 2^32 + xf, a 64-bit fixed-point number of periods (resolution 2.3e-10 L), changed only
+//     by exact integer additions;
+//   * x, a float offset that starts at 0 and collects the increments of at most four steps, so it
+//     is rounded at the magnitude of a few dt v (ulp ~ 1e-9 L), not of the position.
+// After every step whose global index is 3 mod 4 (the end of a Philox block on the fast path; the
+// single-step path applies the same rule, so split launches stay bit-identical) fold() moves the
+// offset into X: rni(x 2^32 / L) by one F2I, IADD3 + IADD3.X, and recomputes thb, the angle of the
+// fraction word (I2F of the signed word: relative 2^-25 of at most half a period).  The force is
+// then cos(thb + (2 pi / L) x): the same FFMA as in fast mode with thb in place of the phase.
+// Cost over fast mode: 2 FP32 + 1 F2I + 1 I2F + 2 integer adds per FOUR steps, two more words of
+// state.  (A float -> integer conversion per step would be cheaper on the FMA port but runs at MUFU
+// rate on the pipe the cosines already keep 60 % busy.)  Valid while 4 |v dt| < L / 2.
 __device__ __forceinline__ float fixed_angle(uint32_t xf, float th_o) {
   // 2 pi 2^-32 * (signed fraction) + phase
   return __fmaf_rn(static_cast<float>(static_cast<int32_t>(xf)), 1.4629180792671596e-09f, th_o);
 }
-__device__ __forceinline__ float force_of_angle(const Coef<float>& k, float th, float k0t) {
-  const float c = fast_cos(th);
-  return __fmaf_rn(__fmaf_rn(k.k2, c, k.k1), c, k0t);
-}
-__device__ __forceinline__ void advance_fixed(State<float>& s, float scaled_increment) {
-  const int32_t d = __float2int_rn(scaled_increment);
+__device__ __forceinline__ void fold(State<float>& s, const Coef<float>& k) {
+  const int32_t d = __float2int_rn(__fmul_rn(s.x, k.fxS));
   const int64_t X = ((static_cast<int64_t>(s.xc) << 32) | s.xf) + static_cast<int64_t>(d);
   s.xf = static_cast<uint32_t>(X);
   s.xc = static_cast<int32_t>(X >> 32);
+  s.x = 0.0f;
+  s.thb = fixed_angle(s.xf, k.th_o);
 }
-// The position the ABI exposes (frames, moments, raster) in precise mode: X L 2^-32 in fp32
-// (X rounded to 24 bits by the conversion, then one multiply).
-__device__ __forceinline__ float position_fixed(uint32_t xf, int32_t xc, float L) {
+__device__ __forceinline__ void fold(State<double>&, const Coef<double>&) {}
+// The position the ABI exposes (frames, moments, raster) in precise mode, in fp32:
+// X rounded to 24 bits by the conversion, times L 2^-32, plus the offset (one FMA).
+__device__ __forceinline__ float position_fixed(uint32_t xf, int32_t xc, float x, float L) {
   const long long X = (static_cast<long long>(xc) << 32) | xf;
-  return __fmul_rn(__ll2float_rn(X), __fmul_rn(L, 0x1p-32f));
+  return __fmaf_rn(__ll2float_rn(X), __fmul_rn(L, 0x1p-32f), x);
 }
 // x[k] of the state arrays as a position (xl == nullptr: the x array holds positions; else the x
-// array holds the bits of xf and the xl array the bits of xc)
-__device__ __forceinline__ float load_position(const float* x, const float* xl, uint64_t k, float L) {
-  return xl ? position_fixed(__float_as_uint(x[k]), __float_as_int(xl[k]), L) : x[k];
+// array holds the offset and the xl / xh arrays the bits of xf / xc)
+__device__ __forceinline__ float load_position(const float* x, const float* xl, const float* xh,
+                                               uint64_t k, float L) {
+  return xl ? position_fixed(__float_as_uint(xl[k]), __float_as_int(xh[k]), x[k], L) : x[k];
 }
-__device__ __forceinline__ double load_position(const double* x, const double*, uint64_t k, double) {
+__device__ __forceinline__ double load_position(const double* x, const double*, const double*,
+                                                uint64_t k, double) {
   return x[k];
 }
 
 template <bool PRECISE, typename Real>
 __device__ __forceinline__ void em_step(State<Real>& s, const Coef<Real>& k, Real k0t, Real rho,
                                         Real cs) {
-  Real f;
-  if constexpr (PRECISE) f = force_of_angle(k, fixed_angle(s.xf, k.th_o), k0t);
-  else f = force<PRECISE>(k, s.x, k0t);
+  const Real f = force<PRECISE>(k, s.x, k0t, s.thb);
   const Real av = fma_(fma_(k.d, s.e, -k.gamma0), s.v, f);
   const Real ae = fma_(-s.e, fma_(k.d, mul_(s.v, s.v), k.c), k.q);
-  if constexpr (PRECISE) advance_fixed(s, mul_(s.v, k.dtS));
-  else s.x = fma_(k.dt, s.v, s.x);
+  s.x = fma_(k.dt, s.v, s.x);
   s.v = fma_(rho, cs, fma_(k.dt, av, s.v));
   s.e = fma_(k.dt, ae, s.e);
 }
@@ -446,30 +449,16 @@ template <bool PRECISE, typename Real>
 __device__ __forceinline__ void heun_step(State<Real>& s, const Coef<Real>& k, Real k0t, Real k0t1,
                                           Real rho, Real cs) {
   const Real sz = mul_(rho, cs);
-  Real f1, th1 = 0;
-  if constexpr (PRECISE) {
-    th1 = fixed_angle(s.xf, k.th_o);
-    f1 = force_of_angle(k, th1, k0t);
-  } else {
-    f1 = force<PRECISE>(k, s.x, k0t);
-  }
+  const Real f1 = force<PRECISE>(k, s.x, k0t, s.thb);
   const Real av1 = fma_(fma_(k.d, s.e, -k.gamma0), s.v, f1);
   const Real ae1 = fma_(-s.e, fma_(k.d, mul_(s.v, s.v), k.c), k.q);
+  const Real xp = fma_(k.dt, s.v, s.x);
   const Real vp = add_(s.v, fma_(k.dt, av1, sz));
   const Real ep = fma_(k.dt, ae1, s.e);
-  Real f2;
-  if constexpr (PRECISE) {
-    // the predicted position enters only through its angle: th1 + (2 pi / L) dt v, rounded at the
-    // magnitude of an angle within a period (no second float -> integer conversion: those run at
-    // MUFU rate on the same pipe as the cosines)
-    f2 = force_of_angle(k, fma_(s.v, mul_(k.dt, k.th_s), th1), k0t1);
-  } else {
-    f2 = force<PRECISE>(k, fma_(k.dt, s.v, s.x), k0t1);
-  }
+  const Real f2 = force<PRECISE>(k, xp, k0t1, s.thb);
   const Real av2 = fma_(fma_(k.d, ep, -k.gamma0), vp, f2);
   const Real ae2 = fma_(-ep, fma_(k.d, mul_(vp, vp), k.c), k.q);
-  if constexpr (PRECISE) advance_fixed(s, mul_(add_(s.v, vp), k.hdtS));
-  else s.x = fma_(k.hdt, add_(s.v, vp), s.x);
+  s.x = fma_(k.hdt, add_(s.v, vp), s.x);
   s.v = add_(s.v, fma_(k.hdt, add_(av1, av2), sz));  // one rounding at the magnitude of v
   s.e = fma_(k.hdt, add_(ae1, ae2), s.e);
 }

@@ -43,7 +43,8 @@ struct StepArgs {
   Real* x;
   Real* v;
   Real* e;
-  Real* xl;                      // high word of the fixed-point position (PRECISE; else nullptr)
+  Real* xl;                      // PRECISE: bits of xf, the fraction word of the fixed-point position
+  Real* xh;                      // PRECISE: bits of xc, its whole periods (else both nullptr)
   const Coef<Real>* coef_table;  // [n_sets] (used when !UNIFORM)
   const Real* tilt;              // tilt[j] = cos(omega (tilt_base + j) dt) (used when TILT)
   void* snap;                    // bound snapshot buffer or nullptr
@@ -108,21 +109,22 @@ __device__ __forceinline__ void store_snapshot(void* snap, uint32_t stride, uint
 template <typename Real>
 __global__ void snapshot_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
                                 const Real* __restrict__ e, const Real* __restrict__ xl,
+                                const Real* __restrict__ xh,
                                 const Coef<Real>* __restrict__ coef_table, uint64_t n_traj,
                                 uint64_t n_particles, uint32_t n_sets, void* snap, uint32_t stride) {
   const uint64_t k = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (k >= n_traj) return;
   const uint32_t set = n_sets == 1 ? 0u : static_cast<uint32_t>(k / n_particles);
-  State<Real> s{load_position(x, xl, k, coef_table[set].L), v[k], e[k], Real(0), 0u, 0};
+  State<Real> s{load_position(x, xl, xh, k, coef_table[set].L), v[k], e[k], Real(0), 0u, 0, Real(0)};
   store_snapshot(snap, stride, k, s);
 }
 
 // ---------------------------------------------------------------------------------------------
 // S0  init
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void store_fixed(float* x, float* xl, uint64_t k, uint32_t xf, int32_t xc) {
-  x[k] = __uint_as_float(xf);
-  xl[k] = __int_as_float(xc);
+__device__ __forceinline__ void store_fixed(float* xl, float* xh, uint64_t k, uint32_t xf, int32_t xc) {
+  xl[k] = __uint_as_float(xf);
+  xh[k] = __int_as_float(xc);
 }
 __device__ __forceinline__ void store_fixed(double*, double*, uint64_t, uint32_t, int32_t) {}
 
@@ -131,15 +133,17 @@ __global__ void init_kernel(Real* __restrict__ x, Real* __restrict__ v, Real* __
                             const Coef<Real>* __restrict__ coef_table, uint64_t n_traj,
                             uint64_t n_particles, uint64_t traj_base, uint64_t set_stride,
                             uint64_t seed, uint32_t n_sets, uint32_t init_v,
-                            uint4* __restrict__ rng_state, Real* __restrict__ xl) {
+                            uint4* __restrict__ rng_state, Real* __restrict__ xl,
+                            Real* __restrict__ xh) {
   const uint64_t k = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (k >= n_traj) return;
   const TrajId id = traj_id(k, n_particles, traj_base, set_stride, n_sets == 1);
   if (rng_state) rng_state[k] = xorshift_seed(seed, id.global);
   const Coef<Real> c = coef_table[id.set];
   const uint4 w = philox_block(seed, id.global, INIT_BLOCK);
-  if (xl) {  // precise fp32 mode: X = x0 2^32 / L = (w0 >> 8) << 8 exactly; the arrays hold its words
-    store_fixed(x, xl, k, w.x & 0xffffff00u, 0);
+  if (xl) {  // precise fp32 mode: X = x0 2^32 / L = (w0 >> 8) << 8 exactly, offset 0
+    store_fixed(xl, xh, k, w.x & 0xffffff00u, 0);
+    x[k] = Real(0);
   } else {
     x[k] = init_x(c, w.x);
   }
@@ -210,13 +214,14 @@ __device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf,
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.sn, t1, t2);
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.cs, t2, t3);
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.sn, t3, t4);
+  if constexpr (PRECISE) fold(s, cf);  // after the step with global index 3 mod 4
 }
 
 // The state as a frame shows it: in precise mode x is the remainder, the frame wants the position.
 template <bool PRECISE, typename Real>
 __device__ __forceinline__ State<Real> frame_state(const State<Real>& s, const Coef<Real>& cf) {
   State<Real> o = s;
-  if constexpr (PRECISE) o.x = position_fixed(s.xf, s.xc, cf.L);
+  if constexpr (PRECISE) o.x = position_fixed(s.xf, s.xc, s.x, cf.L);
   return o;
 }
 
@@ -381,6 +386,9 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
         if (INTEG == 1) t1 = a.tilt[n - a.tilt_base + 1];
       }
       one_step<Real, INTEG, TILT, PRECISE>(s, cf, rho, cs, t0, t1);
+      if constexpr (PRECISE) {
+        if ((n & 3u) == 3u) fold(s, cf);  // the same rule as four_steps
+      }
       ++n;
     }
     if (n == next_snap) {
@@ -415,10 +423,11 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
     cf.bm_o = g->bm_o;
   }
 
-  State<Real> s{a.x[k], a.v[k], a.e[k], Real(0), 0u, 0};
-  if constexpr (PRECISE) {  // the arrays hold the two words of the fixed-point position
-    s.xf = __float_as_uint(a.x[k]);
-    s.xc = __float_as_int(a.xl[k]);
+  State<Real> s{a.x[k], a.v[k], a.e[k], Real(0), 0u, 0, Real(0)};
+  if constexpr (PRECISE) {  // x is the offset; the xl / xh arrays hold the fixed-point words
+    s.xf = __float_as_uint(a.xl[k]);
+    s.xc = __float_as_int(a.xh[k]);
+    s.thb = fixed_angle(s.xf, cf.th_o);
   }
 
   // High word of the global trajectory index (Philox counter word 3): the host passes it as a
@@ -438,8 +447,8 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
   }
 
   if (active) {
-    if constexpr (PRECISE) store_fixed(a.x, a.xl, k, s.xf, s.xc);
-    else a.x[k] = s.x;
+    if constexpr (PRECISE) store_fixed(a.xl, a.xh, k, s.xf, s.xc);
+    a.x[k] = s.x;
     a.v[k] = s.v;
     a.e[k] = s.e;
     if (XS) a.rng_state[k] = S;
@@ -456,7 +465,7 @@ template <typename Real>
 __global__ void __launch_bounds__(MOM_BLOCK)
 moments_partial_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
                        const Real* __restrict__ e, const Real* __restrict__ xl,
-                       const Coef<Real>* __restrict__ coef_table,
+                       const Real* __restrict__ xh, const Coef<Real>* __restrict__ coef_table,
                        uint64_t n_particles, uint64_t traj_base, uint64_t set_stride, uint64_t seed,
                        uint32_t blocks_per_set, uint32_t slice, double* __restrict__ partial) {
   const uint32_t set = blockIdx.x / blocks_per_set;
@@ -470,7 +479,7 @@ moments_partial_kernel(const Real* __restrict__ x, const Real* __restrict__ v,
     const uint64_t k = static_cast<uint64_t>(set) * n_particles + r;
     const uint64_t g = traj_base + static_cast<uint64_t>(set) * set_stride + r;
     const uint4 w = philox_block(seed, g, INIT_BLOCK);
-    const double xi = static_cast<double>(load_position(x, xl, k, c.L));
+    const double xi = static_cast<double>(load_position(x, xl, xh, k, c.L));
     const double vi = static_cast<double>(v[k]);
     const double dx = xi - static_cast<double>(init_x(c, w.x));
     acc[0] += xi;
@@ -586,7 +595,7 @@ __device__ __forceinline__ uint32_t raster_bin(double x, double v, double L, dou
 template <typename Real, bool SMEM>
 __global__ void __launch_bounds__(RASTER_BLOCK)
 raster_kernel(const Real* __restrict__ x, const Real* __restrict__ v, const Real* __restrict__ xl,
-              const Coef<Real>* __restrict__ coef_table, uint64_t n_traj, uint64_t n_particles,
+              const Real* __restrict__ xh, const Coef<Real>* __restrict__ coef_table, uint64_t n_traj, uint64_t n_particles,
               uint32_t n_sets, uint32_t W, uint32_t H, double v_min, double v_range,
               uint32_t* __restrict__ counts) {
   extern __shared__ uint32_t hist[];
@@ -601,7 +610,7 @@ raster_kernel(const Real* __restrict__ x, const Real* __restrict__ v, const Real
     const uint32_t set = n_sets == 1 ? 0u : static_cast<uint32_t>(k / n_particles);
     const Real Lr = coef_table[set].L;
     const double L = static_cast<double>(Lr);
-    const uint32_t bin = raster_bin(static_cast<double>(load_position(x, xl, k, Lr)),
+    const uint32_t bin = raster_bin(static_cast<double>(load_position(x, xl, xh, k, Lr)),
                                     static_cast<double>(v[k]), L, v_min,
                                     v_range, W, H);
     if (bin != 0xffffffffu) {
