@@ -303,7 +303,9 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
           }
         } while (left);
         n += static_cast<uint64_t>(nb) << 2;
-        if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
+        // aligned K: the frames of this run were stored above.  Otherwise the run ended at or before
+        // the next frame, which the check at the bottom of the loop stores.
+        if (K && snap_aligned) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
       } else {
       uint4 w = philox4x32_10(b_lo, b_hi, traj_lo, traj_hi, k0, k1);
       if (TABLE) {
@@ -361,7 +363,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
         } while (left);
       }
       n += static_cast<uint64_t>(nb) << 2;
-      if (K) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
+      if (K && snap_aligned) next_snap = (n / K + 1) * static_cast<uint64_t>(K);
       }
     } else {
       // ---- slow path: one step (unaligned head / tail, or K not a multiple of 4) ----

@@ -225,6 +225,25 @@ def test_snapshot_frame_semantics(abm, torch, with_e):
         assert np.array_equal(frame.cpu().numpy(), f)   # unbound: frame no longer touched
 
 
+@pytest.mark.parametrize("K,steps", [(1, 9), (6, 61), (7, 49), (10, 100), (10, 95), (12, 48), (100, 250), (3, 2)])
+@pytest.mark.parametrize("rng", [0, 1])
+def test_snapshot_every_K_holds_the_last_multiple_of_K(abm, torch, K, steps, rng):
+    """Any K (multiple of 4 or not), any step count: after abm_step the bound buffer holds the state at the last
+    step index that is a multiple of K (one frame, overwritten; reading G20)."""
+    wl = W.config0()
+    p = [dict(wl.set_params(0), rng=rng)]
+    with abm.Ensemble(p, 700, wl.seed, snapshot_every=K) as ens, abm.Ensemble(p, 700, wl.seed) as ref:
+        frame = ens.bind_snapshot()
+        ens.step(steps)
+        ref.step(steps - steps % K)
+        torch.cuda.synchronize()
+        assert np.array_equal(frame.cpu().numpy().astype(np.float64), ref.state()[:, :2])
+        ens.step(K + 1)                                   # a second launch starting off the frame grid
+        ref.step((steps + K + 1) // K * K - (steps - steps % K))
+        torch.cuda.synchronize()
+        assert np.array_equal(frame.cpu().numpy().astype(np.float64), ref.state()[:, :2])
+
+
 def test_snapshot_argument_checks(abm, torch):
     wl = W.config0()
     with abm.Ensemble([wl.set_params(0)], 64, 1) as ens:
@@ -517,3 +536,48 @@ def test_xorshift_split_launches_are_bit_identical(abm, torch, mk, n, K):
     with abm.Ensemble([dict(p, rng=0)], n, wl.seed) as c:
         c.step(72)
         assert not np.array_equal(c.state(), sa)
+
+
+# ---------------------------------------------------------------------------------------------
+# accuracy modes: PRECISE (fixed-point position + four-step offset) on every integrator
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("mk,over", [(W.config0, {}), (W.config1, dict(F0=-2.0)), (W.config3, {}),
+                                     (W.config3, dict(L=0.5, phi=0.1)), (W.config0, dict(L=3.0, A1=-0.7))],
+                         ids=["em", "em_loaded", "heun_tilt", "heun_L0.5", "em_L3"])
+def test_precise_mode_state_frames_moments_and_splits(abm, torch, oracle, mk, over):
+    wl = mk()
+    p = dict(wl.set_params(0), **over)
+    n, K = 1000, 10
+    with abm.Ensemble([p], n, wl.seed, snapshot_every=K, accuracy=abm.ABM_ACCURACY_PRECISE) as a, \
+            abm.Ensemble([p], n, wl.seed, snapshot_every=K, accuracy=abm.ABM_ACCURACY_PRECISE) as b, \
+            abm.Ensemble([p], n, wl.seed, accuracy=abm.ABM_ACCURACY_FAST) as fast:
+        assert a.accuracy == abm.ABM_ACCURACY_PRECISE and fast.accuracy == abm.ABM_ACCURACY_FAST
+        x0 = oracle.init_many(p, wl.seed, n)[0]
+        assert np.array_equal(a.state()[:, 0], x0.astype(np.float32).astype(np.float64))   # init is exact
+        fa, fb = a.bind_snapshot(with_e=True), b.bind_snapshot(with_e=True)
+        a.step(100)
+        for part in (1, 2, 3, 5, 4, 7, 8, 13, 18, 39):       # 100 steps through every block phase
+            b.step(part)
+        got, got_b = a.state(), b.state()
+        assert np.array_equal(got, got_b)                     # split launches: bit-identical
+        torch.cuda.synchronize()
+        assert torch.equal(fa, fb)
+        assert np.array_equal(fa.cpu().numpy()[:, :3].astype(np.float64), got)   # frame == state at a multiple of K
+        x, v, e = oracle.init_many(p, wl.seed, n)
+        oracle.run(p, wl.seed, x, v, e, 0, 100)
+        want = np.stack([x, v, e], 1)
+        err = scale_rel_err(got, want)
+        fast.step(100)
+        err_fast = scale_rel_err(fast.state(), want)
+        print(f"precise {err}  fast {err_fast}")
+        assert np.all(err <= TOL_F32), err
+        assert err[0] <= err_fast[0] * 1.05                   # never worse in x than the fast mode
+        m = a.moments()[0]
+        x0_f32 = x0.astype(np.float32).astype(np.float64)     # dx is taken against the fp32 initial state
+        om = oracle.moments(got[:, 0].copy(), got[:, 1].copy(), got[:, 2].copy(), x0_f32)
+        for k_, val in om.items():
+            assert m[k_] == pytest.approx(val, rel=1e-9, abs=1e-12), k_
+        counts, _ = a.raster(64, 32, -3.0, 3.0)
+        torch.cuda.synchronize()
+        assert np.array_equal(counts.cpu().numpy().view(np.uint32), oracle.raster(got[:, 0], got[:, 1], p["L"], 64, 32, -3.0, 3.0))
