@@ -581,3 +581,44 @@ def test_precise_mode_state_frames_moments_and_splits(abm, torch, oracle, mk, ov
         counts, _ = a.raster(64, 32, -3.0, 3.0)
         torch.cuda.synchronize()
         assert np.array_equal(counts.cpu().numpy().view(np.uint32), oracle.raster(got[:, 0], got[:, 1], p["L"], 64, 32, -3.0, 3.0))
+
+
+# ---------------------------------------------------------------------------------------------
+# every kernel instantiation once: precision x integrator x tilt x (one | several sets) x generator
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("rng", [0, 1], ids=["philox", "xorshift"])
+@pytest.mark.parametrize("n_sets", [1, 3], ids=["oneset", "sets"])
+@pytest.mark.parametrize("tilt", [0.0, 0.4], ids=["notilt", "tilt"])
+@pytest.mark.parametrize("integrator", [0, 1], ids=["em", "heun"])
+@pytest.mark.parametrize("precision", [0, 1], ids=["f32", "f64"])
+def test_kernel_matrix_against_the_oracle(abm, oracle, precision, integrator, tilt, n_sets, rng):
+    base = dict(W.DEFAULTS, precision=precision, integrator=integrator, A=tilt, omega=2.3, F0=0.15, rng=rng,
+                dt=2e-3, init_v=1)
+    sets = [dict(base, D=0.05 + 0.1 * s, q=1.0 + 0.25 * s, L=1.0 + 0.5 * s) for s in range(n_sets)]
+    n, steps, seed = 203, 50, 2718                      # ragged: one CTA + 75 threads per set
+    for acc in ([abm.ABM_ACCURACY_FAST, abm.ABM_ACCURACY_PRECISE] if precision == 0 else [abm.ABM_ACCURACY_AUTO]):
+        with abm.Ensemble(sets, n, seed, accuracy=acc) as ens:
+            ens.step(steps)
+            got = ens.state().reshape(n_sets, n, 3)
+            m = ens.moments()
+        for s, p in enumerate(sets):
+            x, v, e = oracle.init_many(p, seed, n, s * n)
+            oracle.run(p, seed, x, v, e, 0, steps, s * n)
+            err = scale_rel_err(got[s], np.stack([x, v, e], 1))
+            assert np.all(err <= (TOL_F32 if precision == 0 else TOL_F64)), (acc, s, err)
+            assert m["mean_v"][s] == pytest.approx(got[s][:, 1].mean(), rel=1e-9, abs=1e-12)
+
+
+def test_trajectory_index_beyond_32_bits(abm, oracle):
+    """Global indices that straddle a multiple of 2^32 (Philox counter word 3 differs inside one launch:
+    the kernel must not use the shared block-head table) and sit above it."""
+    wl = W.config0()
+    p = wl.set_params(0)
+    for base in (2**32 - 100, 5 * 2**32 + 7):
+        with abm.Ensemble([p], 300, wl.seed, traj_base=base) as ens:
+            ens.step(40)
+            got = ens.state()
+        x, v, e = oracle.init_many(p, wl.seed, 300, base)
+        oracle.run(p, wl.seed, x, v, e, 0, 40, base)
+        assert np.all(scale_rel_err(got, np.stack([x, v, e], 1)) <= TOL_F32)
