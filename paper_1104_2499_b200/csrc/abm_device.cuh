@@ -238,19 +238,18 @@ __device__ __forceinline__ Normal2f box_muller_f32(uint32_t wa, uint32_t wb, flo
 // takes no 64-bit immediate), quadrant selects and special-case branches than on DFMAs, and the
 // fp64 kernel was issue-bound by them.  Here: t is reduced to r = t - rint(t) in [-1/2, 1/2]
 // (magic-number rounding, exact), the parity of rint(t) goes to the sign bit with two integer
-// instructions, and cos(pi r) / sin(pi r) are Taylor polynomials in r^2 whose coefficients
-// (-1)^k pi^2k / (2k)!, (-1)^k pi^(2k+1) / (2k+1)!, k <= 10 sit in constant memory, which DFMA
-// reads as an operand.  Truncation (pi/2)^22 / 22! = 2e-17; measured max abs error 3.3e-16.
+// instructions, and cos(pi r), sin(pi r) / r are degree-8 polynomials in r^2 (Chebyshev fits on
+// r^2 in [0, 1/4], approximation error 4e-18 and 7e-19) whose coefficients sit in constant memory,
+// which DFMA reads as an operand.  Measured max abs error 3.3e-16 (rounding).
 // Valid for |t| < 2^51.
 // ---------------------------------------------------------------------------------------------
-__constant__ double C_COSPI[11] = {
-    1.0, -4.934802200544679, 4.0587121264167685, -1.3352627688545895, 0.2353306303588932,
-    -0.02580689139001406, 0.0019295743094039231, -0.0001046381049248457, 4.303069587032947e-06,
-    -1.3878952462213771e-07, 3.604730797462501e-09};
-__constant__ double C_SINPI[11] = {
-    3.141592653589793, -5.16771278004997, 2.5501640398773455, -0.5992645293207921,
-    0.08214588661112823, -0.0073704309457143504, 0.00046630280576761255, -2.1915353447830217e-05,
-    7.952054001475513e-07, -2.2948428997269873e-08, 5.392664662608129e-10};
+__constant__ double C_COSPI[9] = {
+    1.0, -4.934802200544676, 4.058712126416497, -1.335262768843447, 0.23533063012953284,
+    -0.025806888737002202, 0.0019295562724817132, -0.00010456655338748738, 4.149564353942586e-06};
+__constant__ double C_SINPI[9] = {
+    3.141592653589793, -5.167712780049969, 2.5501640398773007, -0.5992645293189447,
+    0.0821458865731029, -0.007370430505916944, 0.0004662998161898394, -2.1903497074626018e-05,
+    7.697826768224191e-07};
 
 __device__ __forceinline__ double reduce_half_turns(double t, uint32_t& sign) {
   const double magic = 6755399441055744.0;  // 1.5 * 2^52: adding it rounds to an integer
@@ -265,18 +264,22 @@ __device__ __forceinline__ double cospi_f64(double t) {
   uint32_t sign;
   const double r = reduce_half_turns(t, sign);
   const double r2 = __dmul_rn(r, r);
-  double p = C_COSPI[10];
+  double p = C_COSPI[8];
 #pragma unroll
-  for (int k = 9; k >= 0; --k) p = __fma_rn(p, r2, C_COSPI[k]);
+  for (int k = 7; k >= 0; --k) p = __fma_rn(p, r2, C_COSPI[k]);
   return flip_sign(p, sign);
 }
-__device__ __forceinline__ void sincospi_f64(double t, double* sn, double* cs) {
-  uint32_t sign;
-  const double r = reduce_half_turns(t, sign);
+// cos(pi t), sin(pi t) for t = 2 u, u = (w + 1/2) 2^-32 (the Box-Muller angle): rint(t) and the
+// remainder come from the integer w exactly -- n = (w + 2^30) >> 31, r = (int32(w - n 2^31) + 1/2) 2^-31.
+__device__ __forceinline__ void sincospi_2u_f64(uint32_t w, double* sn, double* cs) {
+  const uint32_t n = (w >> 31) + ((w >> 30) & 1u);  // = (w + 2^30) >> 31 without the overflow
+  const int32_t d = static_cast<int32_t>(w - (n << 31));
+  const uint32_t sign = n << 31;                    // parity of n -> sign bit
+  const double r = __fma_rn(static_cast<double>(d), 0x1p-31, 0x1p-32);  // exact
   const double r2 = __dmul_rn(r, r);
-  double p = C_COSPI[10], q = C_SINPI[10];
+  double p = C_COSPI[8], q = C_SINPI[8];
 #pragma unroll
-  for (int k = 9; k >= 0; --k) {
+  for (int k = 7; k >= 0; --k) {
     p = __fma_rn(p, r2, C_COSPI[k]);
     q = __fma_rn(q, r2, C_SINPI[k]);
   }
@@ -286,12 +289,13 @@ __device__ __forceinline__ void sincospi_f64(double t, double* sn, double* cs) {
 
 // -2 ln u for u = (w + 1/2) 2^-32 = k 2^-33, k = 2w + 1, without the math library (same reason):
 // k = m 2^e with m in [sqrt(1/2), sqrt(2)) by integer surgery on the exponent field, s = (m - 1) /
-// (m + 1) by two Newton steps on a single-precision reciprocal plus one residual correction,
-// ln m = 2 atanh s = s sum_j 2/(2j+1) s^2j (|s| <= 0.1716, 11 terms, truncation 6e-19), and
+// (m + 1) by one Newton step on a single-precision reciprocal plus one residual correction,
+// ln m = 2 atanh s = s P(s^2) (|s| <= 0.1716; P a degree-7 Chebyshev fit, error 2e-18), and
 // ln u = (e - 33) ln 2 + ln m.  The sqrt(2) split keeps the two terms from cancelling as u -> 1.
 // Measured against 40-digit arithmetic: relative error <= 4.2e-16.
-__constant__ double C_ATANH2[11] = {2.0, 2.0 / 3, 2.0 / 5, 2.0 / 7, 2.0 / 9, 2.0 / 11, 2.0 / 13,
-                                    2.0 / 15, 2.0 / 17, 2.0 / 19, 2.0 / 21};
+__constant__ double C_ATANH2[8] = {2.0, 0.6666666666666765, 0.3999999999929671, 0.2857142876191665,
+                                   0.22222196920578138, 0.1818363908063474, 0.15312330090369042,
+                                   0.1481178026103594};
 __device__ __forceinline__ float rcp_approx_f32(float x) {
   float y;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -311,23 +315,21 @@ __device__ __forceinline__ double neg2_ln_uniform_f64(uint32_t w) {
   const double E = static_cast<double>((hi >> 20) - 1023 + adj - 33);
   const double f = __dadd_rn(m, -1.0), g = __dadd_rn(m, 1.0);
   double y = static_cast<double>(rcp_approx_f32(static_cast<float>(g)));
-  y = __fma_rn(y, __fma_rn(-g, y, 1.0), y);
-  y = __fma_rn(y, __fma_rn(-g, y, 1.0), y);
+  y = __fma_rn(y, __fma_rn(-g, y, 1.0), y);  // 2^-23 -> 2^-46; the residual step below squares it again
   double q = __dmul_rn(f, y);
   q = __fma_rn(__fma_rn(-g, q, f), y, q);
   const double q2 = __dmul_rn(q, q);
-  double p = C_ATANH2[10];
+  double p = C_ATANH2[7];
 #pragma unroll
-  for (int j = 9; j >= 0; --j) p = __fma_rn(p, q2, C_ATANH2[j]);
+  for (int j = 6; j >= 0; --j) p = __fma_rn(p, q2, C_ATANH2[j]);
   const double ln_u = __fma_rn(E, 0.6931471805599453, __dmul_rn(q, p));
   return __dmul_rn(-2.0, ln_u);
 }
-// sqrt(a) for a normal positive a: single-precision rsqrt seed, two Newton steps, one residual
+// sqrt(a) for a normal positive a: single-precision rsqrt seed, one Newton step, one residual
 // correction (relative error <= 2.3e-16 measured).
 __device__ __forceinline__ double sqrt_pos_f64(double a) {
   double y = static_cast<double>(rsqrt_approx_f32(static_cast<float>(a)));
   const double h = __dmul_rn(0.5, a);
-  y = __fma_rn(y, __fma_rn(-h, __dmul_rn(y, y), 0.5), y);
   y = __fma_rn(y, __fma_rn(-h, __dmul_rn(y, y), 0.5), y);
   const double g = __dmul_rn(a, y);
   return __fma_rn(__fma_rn(-g, g, a), __dmul_rn(0.5, y), g);
@@ -345,7 +347,7 @@ __device__ __forceinline__ double uniform_f64(uint32_t w) {
 __device__ __forceinline__ Normal2d box_muller_f64(uint32_t wa, uint32_t wb, double sigma) {
   Normal2d o;
   o.rho = __dmul_rn(sigma, sqrt_pos_f64(neg2_ln_uniform_f64(wa)));
-  sincospi_f64(__dmul_rn(2.0, uniform_f64(wb)), &o.sn, &o.cs);
+  sincospi_2u_f64(wb, &o.sn, &o.cs);
   return o;
 }
 
