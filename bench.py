@@ -189,9 +189,15 @@ def run_ours(args, wl, cfg_id):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference "
                          "for the oracle)")
-    torch.cuda.set_device(local_rank)
+    torch.cuda.set_device(local_rank % torch.cuda.device_count())
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        else:   # gloo: exercises the multi-rank flow where ranks must share one GPU (NCCL refuses that)
+            dist.init_process_group("gloo")
+    coll_dev = "cuda" if args.backend == "nccl" else "cpu"
+    if world > 1 and args.backend != "nccl":
+        torch.cuda.set_device(local_rank % torch.cuda.device_count())
     abm.lib()
 
     stream = torch.cuda.Stream()
@@ -233,7 +239,7 @@ def run_ours(args, wl, cfg_id):
                     ev[j][1].record(stream)
                 launches["n"] += step_launches
                 if world > 1:                                                  # S6 (2 kernels) + NCCL
-                    m = sharding.reduce_moments(ens.moment_sums(sums_out), ens.step_count, plan, device="cuda")
+                    m = sharding.reduce_moments(ens.moment_sums(sums_out), ens.step_count, plan, device=coll_dev)
                 else:
                     m = ens.moments(mom_out)                                   # S6 (2 kernels)
                 launches["n"] += 2
@@ -261,7 +267,7 @@ def run_ours(args, wl, cfg_id):
     launches["n"] = 0
     barrier()
     wall0 = time.perf_counter()
-    with ClockSampler(local_rank) as clk:
+    with ClockSampler(torch.cuda.current_device()) as clk:
         for i in range(args.steps):
             flush.fill_(i & 0xff)                       # L2 flush between timed iterations
             torch.cuda.synchronize()
@@ -283,7 +289,7 @@ def run_ours(args, wl, cfg_id):
     barrier()
     t_e2e = time.perf_counter() - t0
 
-    tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device="cuda")
+    tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=coll_dev)
     if world > 1:
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
     t_dev, t_e2e = float(tt[0]), float(tt[1])
@@ -356,6 +362,8 @@ def main():
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="collective backend for N > 1 (gloo only to rehearse the flow with ranks sharing a GPU)")
     ap.add_argument("--rng", default="philox", choices=["philox", "xorshift"],
                     help="generator A/B (SURVEY.md 8(f) NEXT-4); the headline and the roofline are Philox")
     ap.add_argument("--sim-steps", type=int, default=0, help="override the config's step count")

@@ -622,3 +622,30 @@ def test_trajectory_index_beyond_32_bits(abm, oracle):
         x, v, e = oracle.init_many(p, wl.seed, 300, base)
         oracle.run(p, wl.seed, x, v, e, 0, 40, base)
         assert np.all(scale_rel_err(got, np.stack([x, v, e], 1)) <= TOL_F32)
+
+
+def test_tilt_table_across_launch_chunks(abm):
+    """A tilted run is split into launches of at most 65,536 steps, each with its own table of cos(omega t_n).
+    With no potential, no depot coupling and no noise, Euler-Maruyama for dv = (-gamma0 v + A cos(omega t)) dt is a
+    linear recursion whose exact solution (a geometric sum) pins every table entry's phase across the chunk
+    boundary; abm_step(70,000) must also equal abm_step(65,536) + abm_step(4,464) bit for bit."""
+    dt, g, A, om = 1e-3, 2.0, 0.7, 1.3
+    p = dict(W.DEFAULTS, precision=1, A1=0.0, A2=0.0, d=0.0, D=0.0, q=0.0, c=0.0, gamma0=g, A=A, omega=om, dt=dt,
+             v0=0.25)
+    n_steps = 70_000
+    with abm.Ensemble([p], 40, 3) as a, abm.Ensemble([p], 40, 3) as b:
+        a.step(n_steps)
+        b.step(65_536)
+        b.step(4_464)
+        sa = a.state()
+        assert np.array_equal(sa, b.state())
+    # exact solution of the recursion v_{n+1} = (1 - g dt) v_n + A dt cos(om n dt):
+    #   v_N = r^N v_0 + A dt Re[ (z^N - r^N) / (z - r) ],  r = 1 - g dt,  z = exp(i om dt)
+    r, z = 1.0 - g * dt, np.exp(1j * om * dt)
+    want = r**n_steps * 0.25 + A * dt * ((z**n_steps - r**n_steps) / (z - r)).real
+    assert np.allclose(sa[:, 1], want, rtol=0, atol=1e-11)
+    for fp32_steps in (66_000,):                       # the fp32 kernels share the chunking code
+        with abm.Ensemble([dict(p, precision=0)], 40, 3) as c:
+            c.step(fp32_steps)
+            want32 = r**fp32_steps * 0.25 + A * dt * ((z**fp32_steps - r**fp32_steps) / (z - r)).real
+            assert np.allclose(c.state()[:, 1], want32, rtol=0, atol=2e-4)
