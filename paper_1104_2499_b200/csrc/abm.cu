@@ -5,6 +5,7 @@
 // stream.  There is no CPU fallback: every step of the path runs in those kernels.
 #include "abm.h"
 
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -118,6 +119,32 @@ double stiffness(const abm_params& p) {
   return p.dt * g * g * (std::fabs(p.A1) + 4.0 * std::fabs(p.A2));
 }
 
+// Host loops over parameter sets (validation, coefficient precomputation): a sweep has up to 2^16 sets
+// and the device idles meanwhile, so large tables are split over a few host threads.
+template <typename F>
+void parallel_sets(uint32_t n_sets, F&& body) {
+  unsigned n_thr = std::thread::hardware_concurrency();
+  if (n_thr > 8) n_thr = 8;
+  if (n_sets < 8192 || n_thr < 2) {
+    body(0u, n_sets);
+    return;
+  }
+  std::vector<std::thread> pool;
+  const uint32_t chunk = (n_sets + n_thr - 1) / n_thr;
+  try {
+    for (uint32_t s0 = chunk; s0 < n_sets; s0 += chunk)
+      pool.emplace_back([&body, s0, chunk, n_sets] { body(s0, s0 + chunk < n_sets ? s0 + chunk : n_sets); });
+  } catch (...) {  // could not start (more) threads: the rest runs here
+    const uint32_t started = static_cast<uint32_t>(pool.size());
+    for (auto& t : pool) t.join();
+    body(0u, chunk < n_sets ? chunk : n_sets);
+    if ((started + 1) * chunk < n_sets) body((started + 1) * chunk, n_sets);
+    return;
+  }
+  body(0u, chunk < n_sets ? chunk : n_sets);
+  for (auto& t : pool) t.join();
+}
+
 bool finite_all(const abm_params& p) {
   const double v[] = {p.dt, p.gamma0, p.q, p.c, p.d, p.D, p.F0, p.A, p.omega,
                       p.L,  p.A1,     p.A2, p.phi, p.v0, p.e0};
@@ -133,18 +160,24 @@ int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets) {
   if (p0.precision > ABM_FP64 || p0.integrator > ABM_HEUN || p0.init_v > ABM_INIT_V_THERMAL ||
       p0.accuracy > ABM_ACCURACY_PRECISE || p0.rng > ABM_RNG_XORSHIFT128)
     return ABM_EINVAL;
-  for (uint32_t s = 0; s < n_sets; ++s) {
-    const abm_params& p = params[s];
-    if (p.struct_size != sizeof(abm_params) || p.reserved != 0) return ABM_EINVAL;
-    if (p.precision != p0.precision || p.integrator != p0.integrator || p.init_v != p0.init_v ||
-        p.accuracy != p0.accuracy || p.rng != p0.rng || p.snapshot_every != p0.snapshot_every || p.dt != p0.dt || p.omega != p0.omega ||
-        p.traj_base != p0.traj_base || p.traj_set_stride != p0.traj_set_stride ||
-        p.stream != p0.stream)
-      return ABM_EINVAL;
-    if (!finite_all(p)) return ABM_EINVAL;
-    if (!(p.dt > 0.0) || !(p.L > 0.0) || p.D < 0.0) return ABM_EINVAL;
-    if (p.init_v == ABM_INIT_V_THERMAL && !(p.gamma0 > 0.0)) return ABM_EINVAL;
-  }
+  std::atomic<int> bad{0};
+  parallel_sets(n_sets, [&](uint32_t s0, uint32_t s1) {
+    for (uint32_t s = s0; s < s1; ++s) {
+      const abm_params& p = params[s];
+      bool ok = p.struct_size == sizeof(abm_params) && p.reserved == 0;
+      ok = ok && p.precision == p0.precision && p.integrator == p0.integrator && p.init_v == p0.init_v &&
+           p.accuracy == p0.accuracy && p.rng == p0.rng && p.snapshot_every == p0.snapshot_every &&
+           p.dt == p0.dt && p.omega == p0.omega && p.traj_base == p0.traj_base &&
+           p.traj_set_stride == p0.traj_set_stride && p.stream == p0.stream;
+      ok = ok && finite_all(p) && p.dt > 0.0 && p.L > 0.0 && !(p.D < 0.0);
+      ok = ok && !(p.init_v == ABM_INIT_V_THERMAL && !(p.gamma0 > 0.0));
+      if (!ok) {
+        bad.store(1, std::memory_order_relaxed);
+        return;
+      }
+    }
+  });
+  if (bad.load()) return ABM_EINVAL;
   // total trajectory count must fit the kernels' 64-bit indexing and 31-bit grids
   const uint64_t max_traj = static_cast<uint64_t>(0x7fffffffu) * STEP_BLOCK;
   if (n_particles > max_traj / n_sets) return ABM_EINVAL;
@@ -201,32 +234,6 @@ void free_all(abm_ctx* c) {
   for (void* p : all) dev_free(c, p);
   std::free(c->host_coefs);
   c->host_coefs = nullptr;
-}
-
-// Host loops over parameter sets (coefficient precomputation): a sweep has up to 2^16 sets and the
-// device idles meanwhile, so large tables are split over a few host threads.
-template <typename F>
-void parallel_sets(uint32_t n_sets, F&& body) {
-  unsigned n_thr = std::thread::hardware_concurrency();
-  if (n_thr > 8) n_thr = 8;
-  if (n_sets < 8192 || n_thr < 2) {
-    body(0u, n_sets);
-    return;
-  }
-  std::vector<std::thread> pool;
-  const uint32_t chunk = (n_sets + n_thr - 1) / n_thr;
-  try {
-    for (uint32_t s0 = chunk; s0 < n_sets; s0 += chunk)
-      pool.emplace_back([&body, s0, chunk, n_sets] { body(s0, s0 + chunk < n_sets ? s0 + chunk : n_sets); });
-  } catch (...) {  // could not start (more) threads: the rest runs here
-    const uint32_t started = static_cast<uint32_t>(pool.size());
-    for (auto& t : pool) t.join();
-    body(0u, chunk < n_sets ? chunk : n_sets);
-    if ((started + 1) * chunk < n_sets) body((started + 1) * chunk, n_sets);
-    return;
-  }
-  body(0u, chunk < n_sets ? chunk : n_sets);
-  for (auto& t : pool) t.join();
 }
 
 template <typename Real>
