@@ -2,6 +2,7 @@
 
     python -m paper_1104_2499_b200.studies scaling      [--out profiles/rNN_scaling]
     python -m paper_1104_2499_b200.studies presentation [--out profiles/rNN_presentation]
+    python -m paper_1104_2499_b200.studies fig2         [--out profiles/rNN_fig2]
 
 scaling       PAPER.md:100-136 (Figs. 3-4): time of one launch against the number of work items, for
               0, 10^3 and 10^4 iterations per launch; 20 launches per size, the last 15 averaged (:100);
@@ -15,7 +16,9 @@ presentation  PAPER.md:138-194 (Tab. 1): what showing a frame costs, in "iterati
               frame (the non-shared buffer, :152-154), text formatting of the copied frame (the gnuplot
               pipe, :144-150; formatting only, nothing is drawn), plus the CUDA rasteriser (abm_raster).
 
-Both write a .csv and a .md (with the command) next to each other.  Timing: CUDA events on the launching
+fig2          PAPER.md:72-74, :94-96 (Fig. 2): the paper's example result, <v> against the opposing force F0.
+
+All write a .csv and a .md (with the command) next to each other.  Timing: CUDA events on the launching
 stream for device work, perf_counter around synchronous host work.
 """
 import argparse
@@ -171,14 +174,50 @@ def presentation(out):
     return rows
 
 
+def fig2(out):
+    """The paper's example plot (Fig. 2): mean velocity against the opposing load F0, averaged
+    over time and launches (:74).  1,024 values of F0 in [-1, 0] x 1,024 realisations on the Eq. 3 potential
+    (h = 1; depot parameters of BASELINE.json configs[0] -- the paper prints none), ten launches of 10^4 iterations
+    (:122); after every launch the running average <x(t) - x(0)> / t of each work item, as the paper's display
+    loop shows it.  The standard error comes from the same device reduction (mean_dx, mean_dx2)."""
+    import torch
+    torch.cuda.set_device(0)
+    stream = torch.cuda.Stream()
+    wl = W.paper_f0_sweep(n_F0=1024, F0_min=-1.0, F0_max=0.0, realisations=1024, n_steps=100_000)
+    sets = [wl.set_params(s) for s in range(wl.n_param_sets)]
+    dt = sets[0]["dt"]
+    cols = []
+    with torch.cuda.stream(stream):
+        ens = abm.Ensemble(sets, wl.n_particles, wl.seed, stream=stream)
+        a, b = _events(torch)
+        a.record(stream)
+        for launch in range(10):
+            ens.step(10_000)
+            cols.append(ens.time_averaged_velocity())
+        b.record(stream)
+        b.synchronize()
+        m = ens.moments()
+        ens.close()
+    t = 100_000 * dt
+    se = np.sqrt(np.maximum(m["mean_dx2"] - m["mean_dx"] ** 2, 0.0) / wl.n_particles) / t
+    with open(out + ".csv", "w") as f:
+        f.write("F0," + ",".join(f"vbar_after_{(k + 1) * 10_000}_steps" for k in range(10)) + ",standard_error\n")
+        for s in range(wl.n_param_sets):
+            f.write(f"{sets[s]['F0']:.6f}," + ",".join(f"{c[s]:.6f}" for c in cols) + f",{se[s]:.6f}\n")
+    print(f"fig2: {wl.n_trajectories} trajectories x 100000 steps in {a.elapsed_time(b):.1f} ms "
+          f"(10 launches + 10 reductions); <v>(F0=-1) = {cols[-1][0]:+.4f}, <v>(F0=0) = {cols[-1][-1]:+.4f} "
+          f"+- {se[-1]:.4f}", flush=True)
+    return [None] * wl.n_param_sets
+
+
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("study", choices=["scaling", "presentation"])
+    ap.add_argument("study", choices=["scaling", "presentation", "fig2"])
     ap.add_argument("--out", default=None)
     args = ap.parse_args()
     out = args.out or f"gpurun_out/{args.study}"
     os.makedirs(os.path.dirname(out) or ".", exist_ok=True)
-    rows = scaling(out) if args.study == "scaling" else presentation(out)
+    rows = {"scaling": scaling, "presentation": presentation, "fig2": fig2}[args.study](out)
     with open(out + ".md", "w") as f:
         f.write(f"# {args.study} study (SURVEY.md 8(f))\n\nCommand (B200, through gpurun):\n\n"
                 f"    python -m paper_1104_2499_b200.studies {args.study} --out {out}\n\n"
