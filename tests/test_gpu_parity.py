@@ -649,3 +649,62 @@ def test_tilt_table_across_launch_chunks(abm):
             c.step(fp32_steps)
             want32 = r**fp32_steps * 0.25 + A * dt * ((z**fp32_steps - r**fp32_steps) / (z - r)).real
             assert np.allclose(c.state()[:, 1], want32, rtol=0, atol=2e-4)
+
+
+# ---------------------------------------------------------------------------------------------
+# randomised differential test: random (seeded) models, sizes, launch splits and frame periods
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("case", range(24))
+def test_random_cases_against_the_oracle(abm, torch, oracle, case):
+    rng = np.random.default_rng(9000 + case)
+    precision = int(rng.integers(0, 2))
+    n_sets = int(rng.choice([1, 1, 2, 5]))
+    base = dict(W.DEFAULTS, precision=precision, integrator=int(rng.integers(0, 2)), rng=int(rng.integers(0, 2)),
+                init_v=int(rng.integers(0, 2)), dt=float(rng.choice([5e-4, 1e-3, 2e-3])),
+                A=float(rng.choice([0.0, 0.3])), omega=float(rng.uniform(0.5, 3.0)),
+                v0=float(rng.uniform(-0.5, 0.5)), e0=float(rng.uniform(0.0, 1.0)))
+    sets = [dict(base, D=float(rng.uniform(0.0, 0.3)), q=float(rng.uniform(0.0, 2.0)), c=float(rng.uniform(0.05, 0.5)),
+                 d=float(rng.uniform(0.0, 1.5)), gamma0=float(rng.uniform(0.5, 2.0)), F0=float(rng.uniform(-0.5, 0.5)),
+                 L=float(rng.choice([0.5, 1.0, 2.0])), A1=float(rng.uniform(-1.0, 1.0)), A2=float(rng.uniform(-0.3, 0.3)),
+                 phi=float(rng.uniform(0.0, 0.5))) for _ in range(n_sets)]
+    n = int(rng.integers(1, 400))
+    K = int(rng.choice([0, 1, 3, 4, 10, 16, 25]))
+    seed = int(rng.integers(0, 2**63))
+    base_idx = int(rng.choice([0, 12345, 2**32 - 50]))
+    acc = int(rng.integers(0, 3))
+    splits = [int(t) for t in rng.integers(1, 40, size=int(rng.integers(1, 6)))]
+    total = sum(splits)
+    with abm.Ensemble(sets, n, seed, snapshot_every=K, traj_base=base_idx, accuracy=acc) as ens, \
+            abm.Ensemble(sets, n, seed, traj_base=base_idx, accuracy=acc) as ref:
+        frame = ens.bind_snapshot(with_e=bool(rng.integers(0, 2))) if K else None
+        for part in splits:
+            ens.step(part)
+        got = ens.state()
+        m = ens.moments()
+        if K:
+            ref.step(total - total % K)
+            torch.cuda.synchronize()
+            cols = frame.shape[1] if frame.shape[1] == 2 else 3
+            assert np.array_equal(frame.cpu().numpy()[:, :cols].astype(np.float64), ref.state()[:, :cols])
+            ref.step(total % K)
+        else:
+            ref.step(total)
+        assert np.array_equal(got, ref.state())                       # independent of splits and of frames
+    got = got.reshape(n_sets, n, 3)
+    tol = (TOL_F32 if precision == 0 else TOL_F64) * max(1.0, total / 100.0)
+    for s, p in enumerate(sets):
+        first = base_idx + s * n
+        x, v, e = oracle.init_many(p, seed, n, first)
+        x0 = x.copy()
+        oracle.run(p, seed, x, v, e, 0, total, first)
+        want = np.stack([x, v, e], 1)
+        if n >= 8:
+            err = scale_rel_err(got[s], want)
+        else:                                  # too few trajectories for an RMS scale: absolute, scale 1
+            err = np.abs(got[s] - want).max(0) / np.maximum(1.0, np.abs(want).max(0))
+        assert np.all(err <= tol), (case, s, err, dict(base, **p))
+        x0f = x0.astype(np.float32).astype(np.float64) if precision == 0 else x0
+        om = oracle.moments(got[s][:, 0].copy(), got[s][:, 1].copy(), got[s][:, 2].copy(), x0f)
+        for k_, val in om.items():
+            assert m[k_][s] == pytest.approx(val, rel=1e-8, abs=1e-10), (case, s, k_)
