@@ -41,6 +41,7 @@ struct abm_ctx {
   bool precise;         // fp32 accuracy mode resolved at create (include/abm.h, abm_params.accuracy)
   uint64_t n_particles, n_traj, seed, step, traj_base, set_stride;
   double dt, omega;
+  double tilt_k0, tilt_A;  // what the tilt table holds: k0 + A cos(omega t) of the one set, or (0, 1)
   size_t real_size;
   void *x, *v, *e;      // state, SoA, Real[n_traj]
   void* xl;             // precise fp32 mode only: fraction word of the fixed-point position, [n_traj]
@@ -313,6 +314,10 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
   a.traj_base = c->traj_base;
   a.set_stride = c->set_stride;
   a.seed = c->seed;
+  for (uint32_t r = 0; r < 10; ++r) {
+    a.rk0[r] = static_cast<uint32_t>(c->seed) + PHILOX_W0 * r;
+    a.rk1[r] = static_cast<uint32_t>(c->seed >> 32) + PHILOX_W1 * r;
+  }
   a.snap_every = c->snap_every;
   a.snap_stride = c->snap_stride;
   a.coef0 = coef0<Real>(c);
@@ -329,7 +334,7 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
     if (c->tilt) {
       const uint32_t n_tab = chunk + 1;  // Heun reads t_{n+1} of the last step
       tilt_kernel<Real><<<(n_tab + 255) / 256, 256, 0, c->stream>>>(
-          static_cast<Real*>(c->tilt_table), c->step, n_tab, c->omega, c->dt);
+          static_cast<Real*>(c->tilt_table), c->step, n_tab, c->omega, c->dt, c->tilt_k0, c->tilt_A);
       ABM_CK(c, cudaGetLastError());
     }
     ABM_CK(c, launch_step<Real>(c, a));
@@ -418,6 +423,9 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   c->tilt = false;
   for (uint32_t s = 0; s < n_param_sets; ++s)
     if (params[s].A != 0.0) c->tilt = true;
+  // single set: the tilt table holds k0 + A cos(omega t) (k0 = (2 pi / L) 2 A2 + F0 as in make_coef)
+  c->tilt_k0 = n_param_sets == 1 ? (6.283185307179586476925286766559 / p0.L) * 2.0 * p0.A2 + p0.F0 : 0.0;
+  c->tilt_A = n_param_sets == 1 ? p0.A : 1.0;
   c->real_size = c->precision == ABM_FP32 ? 4 : 8;
   c->precise = false;
   if (c->precision == ABM_FP32) {

@@ -104,6 +104,17 @@ __device__ __forceinline__ uint4 philox_finish(const PhiloxTraj& t, uint32_t u0,
   return make_uint4(c0, c1, c2, c3);
 }
 
+// The same with the round keys read from host-computed tables (kernel parameters: constant-bank
+// operands of the LOP3s, no uniform registers or in-loop key arithmetic).
+__device__ __forceinline__ uint4 philox_finish_rk(const PhiloxTraj& t, uint32_t u0, uint32_t u1,
+                                                  uint32_t u2, const uint32_t (&rk0)[10],
+                                                  const uint32_t (&rk1)[10]) {
+  uint32_t c0 = u0 ^ t.p1, c1 = u1, c2 = t.p2 ^ u2, c3 = t.p3;
+#pragma unroll
+  for (int r = 2; r < 10; ++r) philox_round(c0, c1, c2, c3, rk0[r], rk1[r]);
+  return make_uint4(c0, c1, c2, c3);
+}
+
 // Stream layout: key = (seed lo, seed hi),
 // ctr = (block lo, block hi, trajectory lo, trajectory hi).
 __device__ __forceinline__ uint4 philox_block(uint64_t seed, uint64_t traj, uint64_t b) {

@@ -46,7 +46,7 @@ struct StepArgs {
   Real* xl;                      // PRECISE: bits of xf, the fraction word of the fixed-point position
   Real* xh;                      // PRECISE: bits of xc, its whole periods (else both nullptr)
   const Coef<Real>* coef_table;  // [n_sets] (used when !UNIFORM)
-  const Real* tilt;              // tilt[j] = cos(omega (tilt_base + j) dt) (used when TILT)
+  const Real* tilt;              // tilt[j] = k0 + A cos(omega (tilt_base + j) dt): (k0, A) of the one set, or (0, 1)
   void* snap;                    // bound snapshot buffer or nullptr
   uint4* rng_state;              // xorshift state per trajectory (used when XS), at a pair boundary
   uint64_t n_traj;               // local trajectories
@@ -60,6 +60,7 @@ struct StepArgs {
   uint32_t snap_stride;          // bytes per trajectory in snap
   uint32_t traj_hi;              // high word of every global trajectory index, if shared
   uint32_t traj_hi_shared;       // 1: all trajectories of the launch share traj_hi
+  uint32_t rk0[10], rk1[10];     // Philox round keys k0 + r W0, k1 + r W1 (host-computed: constant-bank operands)
   Coef<Real> coef0;              // the single set's coefficients (used when UNIFORM)
 };
 
@@ -152,15 +153,17 @@ __global__ void init_kernel(Real* __restrict__ x, Real* __restrict__ v, Real* __
 }
 
 // ---------------------------------------------------------------------------------------------
-// tilt table: tilt[j] = cos(omega * ((base + j) * dt)), evaluated in fp64 (reading G15)
+// tilt table: tilt[j] = k0 + A cos(omega * ((base + j) * dt)), evaluated in fp64 (reading G15).
+// Single-set runs pass the set's (k0, A): the table then holds the whole time-dependent constant of
+// the force and the step kernel adds nothing; sweeps pass (0, 1) and apply each set's A, k0 themselves.
 // ---------------------------------------------------------------------------------------------
 template <typename Real>
 __global__ void tilt_kernel(Real* __restrict__ tilt, uint64_t base, uint32_t n, double omega,
-                            double dt) {
+                            double dt, double k0, double A) {
   const uint32_t j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= n) return;
   const double t = static_cast<double>(base + j) * dt;
-  tilt[j] = static_cast<Real>(cos(omega * t));
+  tilt[j] = static_cast<Real>(k0 + A * cos(omega * t));  // (k0, A) = (0, 1): the cosine itself
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -186,20 +189,22 @@ struct Noise4<double> {
       : a(box_muller_f64(w.x, w.y, k.s2)), b(box_muller_f64(w.z, w.w, k.s2)) {}
 };
 
-template <typename Real, int INTEG, bool TILT, bool PRECISE>
+template <typename Real, int INTEG, int TILT, bool PRECISE>
 __device__ __forceinline__ void one_step(State<Real>& s, const Coef<Real>& k, Real rho, Real cs,
                                          Real t0, Real t1) {
-  const Real k0t = TILT ? fma_(k.A, t0, k.k0) : k.k0;
+  // TILT == 2: the table holds k0 + A cos(omega t) itself (single-set runs, fp64 on the host side of
+  // the rounding); TILT == 1: it holds cos(omega t) and the set's A, k0 are applied here.
+  const Real k0t = TILT == 2 ? t0 : (TILT ? fma_(k.A, t0, k.k0) : k.k0);
   if (INTEG == 0) {
     em_step<PRECISE>(s, k, k0t, rho, cs);
   } else {
-    const Real k0t1 = TILT ? fma_(k.A, t1, k.k0) : k.k0;
+    const Real k0t1 = TILT == 2 ? t1 : (TILT ? fma_(k.A, t1, k.k0) : k.k0);
     heun_step<PRECISE>(s, k, k0t, k0t1, rho, cs);
   }
 }
 
 // Four steps from one Philox block.
-template <typename Real, int INTEG, bool TILT, bool PRECISE>
+template <typename Real, int INTEG, int TILT, bool PRECISE>
 __device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf, const uint4& w,
                                            const Real*& tl) {
   const Noise4<Real> z(w, cf);
@@ -243,12 +248,23 @@ __device__ __forceinline__ State<Real> frame_state(const State<Real>& s, const C
 // and FFMA / MUFU instead of an integer phase followed by a floating-point phase.  The block
 // after the last one of a run is computed and dropped (its counter may wrap: harmless).
 constexpr int PHILOX_CHUNK = STEP_BLOCK;  // table entries per refill = threads per CTA
+#ifndef ABM_UNROLL2
+#define ABM_UNROLL2 1
+#endif
+#ifndef ABM_RK_CONST
+#define ABM_RK_CONST 1
+#endif
+#if ABM_RK_CONST
+#define PHILOX_FINISH(pt, u, a, k0, k1) philox_finish_rk(pt, (u).x, (u).y, (u).z, (a).rk0, (a).rk1)
+#else
+#define PHILOX_FINISH(pt, u, a, k0, k1) philox_finish(pt, (u).x, (u).y, (u).z, k0, k1)
+#endif
 
 //
 // XS (generator variant, NEXT-4): the words come from the trajectory's xorshift state S instead.
 // S always sits at a pair boundary -- before output 2 (n >> 1) -- when a step starts: whole blocks
 // draw four outputs; a single even step draws its pair from a copy, the odd step after it commits.
-template <typename Real, int INTEG, bool TILT, bool PRECISE, bool TABLE, bool XS>
+template <typename Real, int INTEG, int TILT, bool PRECISE, bool TABLE, bool XS>
 __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_t k, const bool active,
                                           const uint32_t traj_lo, const uint32_t traj_hi,
                                           const Coef<Real>& cf, State<Real>& s, uint4& S) {
@@ -323,14 +339,37 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
           do {
             const uint32_t rest = in_chunk - done;
             const uint32_t seg = rest < to_snap ? rest : static_cast<uint32_t>(to_snap);  // >= 1
-            const uint4* const tp_end = tp + seg;
+            // fp32: two blocks per loop trip -- the look-ahead words alternate between two register
+            // sets, so no moves rotate them and the loop overhead is halved (fp64 is short of
+            // registers: one block per trip).
+            if constexpr (sizeof(Real) == 4 && ABM_UNROLL2 != 0) {
+              if (seg & 1u) {
+                const uint4 u = *tp++;
+                const uint4 w_next = PHILOX_FINISH(pt, u, a, k0, k1);
+                four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+                w = w_next;
+              }
+              const uint4* const tp_end = tp + (seg & ~1u);
 #pragma unroll 1
-            do {
-              const uint4 u = *tp;
-              const uint4 w_next = philox_finish(pt, u.x, u.y, u.z, k0, k1);
-              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
-              w = w_next;
-            } while (++tp != tp_end);
+              while (tp != tp_end) {
+                const uint4 ua = tp[0];
+                const uint4 wa = PHILOX_FINISH(pt, ua, a, k0, k1);
+                four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+                const uint4 ub = tp[1];
+                w = PHILOX_FINISH(pt, ub, a, k0, k1);
+                four_steps<Real, INTEG, TILT, PRECISE>(s, cf, wa, tl);
+                tp += 2;
+              }
+            } else {
+              const uint4* const tp_end = tp + seg;
+#pragma unroll 1
+              do {
+                const uint4 u = *tp;
+                const uint4 w_next = PHILOX_FINISH(pt, u, a, k0, k1);
+                four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+                w = w_next;
+              } while (++tp != tp_end);
+            }
             done += seg;
             if (seg == to_snap) {  // a frame is due after this block
               if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
@@ -436,14 +475,15 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
   // kernel parameter when the whole launch shares one value (always, unless the index range
   // straddles a multiple of 2^32); the block-head table of run_steps needs that.
   uint4 S = make_uint4(0u, 0u, 0u, 0u);
+  constexpr int TL = TILT ? (UNIFORM ? 2 : 1) : 0;  // what the tilt table holds (one_step)
   if (XS) {
     S = a.rng_state[k];
-    run_steps<Real, INTEG, TILT, PRECISE, false, true>(a, k, active, 0u, 0u, cf, s, S);
+    run_steps<Real, INTEG, TL, PRECISE, false, true>(a, k, active, 0u, 0u, cf, s, S);
   } else if (a.traj_hi_shared) {
-    run_steps<Real, INTEG, TILT, PRECISE, ABM_PHILOX_TABLE != 0, false>(
+    run_steps<Real, INTEG, TL, PRECISE, ABM_PHILOX_TABLE != 0, false>(
         a, k, active, static_cast<uint32_t>(id.global), a.traj_hi, cf, s, S);
   } else {
-    run_steps<Real, INTEG, TILT, PRECISE, false, false>(
+    run_steps<Real, INTEG, TL, PRECISE, false, false>(
         a, k, active, static_cast<uint32_t>(id.global), static_cast<uint32_t>(id.global >> 32), cf,
         s, S);
   }
