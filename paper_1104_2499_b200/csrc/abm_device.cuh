@@ -249,18 +249,20 @@ __device__ __forceinline__ Normal2f box_muller_f32(uint32_t wa, uint32_t wb, flo
 // takes no 64-bit immediate), quadrant selects and special-case branches than on DFMAs, and the
 // fp64 kernel was issue-bound by them.  Here: t is reduced to r = t - rint(t) in [-1/2, 1/2]
 // (magic-number rounding, exact), the parity of rint(t) goes to the sign bit with two integer
-// instructions, and cos(pi r), sin(pi r) / r are degree-8 polynomials in r^2 (Chebyshev fits on
-// r^2 in [0, 1/4], approximation error 4e-18 and 7e-19) whose coefficients sit in constant memory,
-// which DFMA reads as an operand.  Measured max abs error 3.3e-16 (rounding).
+// instructions, and cos(pi r), sin(pi r) / r are degree-7 polynomials in r^2 (Chebyshev fits on
+// r^2 in [0, 1/4]: 2.0e-15 absolute and 2.4e-16 relative with the rounded coefficients -- chosen
+// against the 1e-12 trajectory tolerance, where a function error enters multiplied by dt or sigma;
+// degree 8 reached 1e-16 for one more DFMA per evaluation) whose coefficients sit in constant
+// memory, which DFMA reads as an operand.
 // Valid for |t| < 2^51.
 // ---------------------------------------------------------------------------------------------
-__constant__ double C_COSPI[9] = {
-    1.0, -4.934802200544676, 4.058712126416497, -1.335262768843447, 0.23533063012953284,
-    -0.025806888737002202, 0.0019295562724817132, -0.00010456655338748738, 4.149564353942586e-06};
-__constant__ double C_SINPI[9] = {
-    3.141592653589793, -5.167712780049969, 2.5501640398773007, -0.5992645293189447,
-    0.0821458865731029, -0.007370430505916944, 0.0004662998161898394, -2.1903497074626018e-05,
-    7.697826768224191e-07};
+constexpr int N_COSPI = 8, N_SINPI = 8;  // terms: degree 7 in r^2
+__constant__ double C_COSPI[N_COSPI] = {
+    0.9999999999999981, -4.934802200543686, 4.058712126333295, -1.3352627661817635,
+    0.23533058831317874, -0.025806531975921563, 0.0019278700526981333, -0.0001004164642205389};
+__constant__ double C_SINPI[N_SINPI] = {
+    3.1415926535897927, -5.1677127800497855, 2.5501640398618677, -0.599264528825224,
+    0.08214587881631043, -0.0073703643265304155, 0.0004659870158043378, -2.113362735205297e-05};
 
 __device__ __forceinline__ double reduce_half_turns(double t, uint32_t& sign) {
   const double magic = 6755399441055744.0;  // 1.5 * 2^52: adding it rounds to an integer
@@ -275,9 +277,9 @@ __device__ __forceinline__ double cospi_f64(double t) {
   uint32_t sign;
   const double r = reduce_half_turns(t, sign);
   const double r2 = __dmul_rn(r, r);
-  double p = C_COSPI[8];
+  double p = C_COSPI[N_COSPI - 1];
 #pragma unroll
-  for (int k = 7; k >= 0; --k) p = __fma_rn(p, r2, C_COSPI[k]);
+  for (int k = N_COSPI - 2; k >= 0; --k) p = __fma_rn(p, r2, C_COSPI[k]);
   return flip_sign(p, sign);
 }
 // cos(pi t), sin(pi t) for t = 2 u, u = (w + 1/2) 2^-32 (the Box-Muller angle): rint(t) and the
@@ -288,9 +290,10 @@ __device__ __forceinline__ void sincospi_2u_f64(uint32_t w, double* sn, double* 
   const uint32_t sign = n << 31;                    // parity of n -> sign bit
   const double r = __fma_rn(static_cast<double>(d), 0x1p-31, 0x1p-32);  // exact
   const double r2 = __dmul_rn(r, r);
-  double p = C_COSPI[8], q = C_SINPI[8];
+  static_assert(N_COSPI == N_SINPI, "one loop for both polynomials");
+  double p = C_COSPI[N_COSPI - 1], q = C_SINPI[N_SINPI - 1];
 #pragma unroll
-  for (int k = 7; k >= 0; --k) {
+  for (int k = N_COSPI - 2; k >= 0; --k) {
     p = __fma_rn(p, r2, C_COSPI[k]);
     q = __fma_rn(q, r2, C_SINPI[k]);
   }
@@ -301,12 +304,13 @@ __device__ __forceinline__ void sincospi_2u_f64(uint32_t w, double* sn, double* 
 // -2 ln u for u = (w + 1/2) 2^-32 = k 2^-33, k = 2w + 1, without the math library (same reason):
 // k = m 2^e with m in [sqrt(1/2), sqrt(2)) by integer surgery on the exponent field, s = (m - 1) /
 // (m + 1) by one Newton step on a single-precision reciprocal plus one residual correction,
-// ln m = 2 atanh s = s P(s^2) (|s| <= 0.1716; P a degree-7 Chebyshev fit, error 2e-18), and
+// ln m = 2 atanh s = s P(s^2) (|s| <= 0.1716; P a degree-6 Chebyshev fit, relative error 2.3e-16), and
 // ln u = (e - 33) ln 2 + ln m.  The sqrt(2) split keeps the two terms from cancelling as u -> 1.
-// Measured against 40-digit arithmetic: relative error <= 4.2e-16.
-__constant__ double C_ATANH2[8] = {2.0, 0.6666666666666765, 0.3999999999929671, 0.2857142876191665,
-                                   0.22222196920578138, 0.1818363908063474, 0.15312330090369042,
-                                   0.1481178026103594};
+// Relative error of the whole function <= 6e-16 (fit + roundings).
+constexpr int N_ATANH2 = 7;  // terms: degree 6 in s^2
+__constant__ double C_ATANH2[N_ATANH2] = {2.0000000000000004, 0.6666666666655292, 0.40000000061741614,
+                                          0.2857141602110767, 0.22223434547517906, 0.18121934431215214,
+                                          0.16837659970680488};
 __device__ __forceinline__ float rcp_approx_f32(float x) {
   float y;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -330,9 +334,9 @@ __device__ __forceinline__ double neg2_ln_uniform_f64(uint32_t w) {
   double q = __dmul_rn(f, y);
   q = __fma_rn(__fma_rn(-g, q, f), y, q);
   const double q2 = __dmul_rn(q, q);
-  double p = C_ATANH2[7];
+  double p = C_ATANH2[N_ATANH2 - 1];
 #pragma unroll
-  for (int j = 6; j >= 0; --j) p = __fma_rn(p, q2, C_ATANH2[j]);
+  for (int j = N_ATANH2 - 2; j >= 0; --j) p = __fma_rn(p, q2, C_ATANH2[j]);
   const double ln_u = __fma_rn(E, 0.6931471805599453, __dmul_rn(q, p));
   return __dmul_rn(-2.0, ln_u);
 }

@@ -197,6 +197,99 @@ void mix(const Dev& d) {
               (wa + wb) * r);
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// Third table: the instruction mix of the fp32 Euler-Maruyama step loop (one Philox block = four
+// steps: 54 FFMA/FMUL/FADD, 6 x (FMUL.RZ + MUFU.COS), 6 more MUFU, 16 x (IMAD.WIDE + LOP3), 8 more
+// ALU-pipe instructions) as a stream of INDEPENDENT chains, 128-thread CTAs as in the step kernel.
+// What this runs at is what the SM can do with that mix when nothing waits on a dependency: the
+// ceiling the step kernel is compared with in DESIGN.md 8.  MODE bit 0: FP32, 1: Philox, 2: MUFU,
+// 3: the extra ALU instructions.
+// ---------------------------------------------------------------------------------------------
+#define PR_FF(r) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(r) : "f"(fb), "f"(fc));
+#define PR_IW(r)                                                                                  \
+  asm volatile("{\n\t.reg .u64 p;\n\t.reg .u32 lo, hi;\n\tmul.wide.u32 p, %0, 0xD2511F53;\n\t"    \
+               "mov.b64 {lo, hi}, p;\n\tlop3.b32 %0, lo, hi, %1, 0x96;\n\t}" : "+r"(r) : "r"(ub));
+#define PR_LX(r) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r) : "r"(ub), "r"(uc));
+#define PR_MC(r) asm volatile("cos.approx.ftz.f32 %0, %0;" : "+f"(r));
+#define PR_ML(r) asm volatile("lg2.approx.ftz.f32 %0, %0;" : "+f"(r));
+#define PR_MS(r) asm volatile("sqrt.approx.ftz.f32 %0, %0;" : "+f"(r));
+#define PR_ME(r) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(r));
+
+template <int MODE>
+__global__ void __launch_bounds__(128) loop_mix_kernel(int iters, const float* __restrict__ in,
+                                                       float* __restrict__ out,
+                                                       long long* __restrict__ cycles) {
+  float f[12], m[8];
+  uint32_t u[8];
+  const float fb = in[0], fc = in[1];
+  const uint32_t ub = __float_as_uint(in[2]) | 1u, uc = __float_as_uint(in[3]);
+#pragma unroll
+  for (int j = 0; j < 12; ++j) f[j] = in[4] + j + threadIdx.x;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    u[j] = ub * (j + 3) + threadIdx.x;
+    m[j] = in[5] + j * 0.1f;
+  }
+  __syncthreads();
+  const long long t0 = clock64();
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {  // half a block per pass
+      if (MODE & 1) { PR_FF(f[0]) PR_FF(f[1]) PR_FF(f[2]) }
+      if (MODE & 2) { PR_IW(u[0]) PR_IW(u[1]) }
+      if (MODE & 4) { PR_MC(m[0]) }
+      if (MODE & 1) { PR_FF(f[3]) PR_FF(f[4]) PR_FF(f[5]) }
+      if (MODE & 2) { PR_IW(u[2]) PR_IW(u[3]) }
+      if (MODE & 4) { PR_MC(m[1]) PR_ML(m[2]) }
+      if (MODE & 1) { PR_FF(f[6]) PR_FF(f[7]) PR_FF(f[8]) PR_FF(f[0]) }
+      if (MODE & 8) { PR_LX(u[4]) PR_LX(u[5]) }
+      if (MODE & 2) { PR_IW(u[0]) PR_IW(u[1]) }
+      if (MODE & 4) { PR_MC(m[3]) PR_MS(m[4]) }
+      if (MODE & 1) { PR_FF(f[9]) PR_FF(f[10]) PR_FF(f[11]) PR_FF(f[1]) PR_FF(f[2]) }
+      if (MODE & 2) { PR_IW(u[2]) PR_IW(u[3]) }
+      if (MODE & 4) { PR_ME(m[5]) }
+      if (MODE & 8) { PR_LX(u[6]) PR_LX(u[7]) }
+      if (MODE & 1) {
+        PR_FF(f[3]) PR_FF(f[4]) PR_FF(f[5]) PR_FF(f[6]) PR_FF(f[7]) PR_FF(f[8])
+        PR_FF(f[9]) PR_FF(f[10]) PR_FF(f[11]) PR_FF(f[0]) PR_FF(f[1]) PR_FF(f[2])
+      }
+    }
+  }
+  const long long t1 = clock64();
+  float acc = 0;
+  uint32_t ua = 0;
+#pragma unroll
+  for (int j = 0; j < 12; ++j) acc += f[j];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    ua ^= u[j];
+    acc += m[j];
+  }
+  if (static_cast<double>(acc) + static_cast<double>(ua) == 12345.0) out[threadIdx.x] = acc;
+  if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
+// -> SM cycles per warp and scheduler for one pass of the mix (one Philox block = four steps)
+template <int MODE>
+double loop_mix(const Dev& d, int ctas_per_sm) {
+  const int iters = 20000, grid = d.n_sm * ctas_per_sm;
+  loop_mix_kernel<MODE><<<grid, 128>>>(200, d.in, d.out, d.cyc);
+  loop_mix_kernel<MODE><<<grid, 128>>>(iters, d.in, d.out, d.cyc);
+  CK(cudaDeviceSynchronize());
+  std::vector<long long> c(grid);
+  CK(cudaMemcpy(c.data(), d.cyc, sizeof(long long) * grid, cudaMemcpyDeviceToHost));
+  const long long worst = *std::max_element(c.begin(), c.end());
+  return static_cast<double>(worst) / iters / ctas_per_sm;  // a CTA has one warp per scheduler
+}
+
+template <int MODE>
+void loop_mix_row(const Dev& d, const char* name) {
+  std::printf("%-44s %8.1f %8.1f %8.1f\n", name, loop_mix<MODE>(d, 4), loop_mix<MODE>(d, 9),
+              loop_mix<MODE>(d, 12));
+}
+
 int main() {
   Dev d;
   cudaDeviceProp p;
@@ -210,7 +303,7 @@ int main() {
   CK(cudaMemcpy(d.in, h_in, sizeof(h_in), cudaMemcpyHostToDevice));
   CK(cudaMemcpyToSymbol(c_k, h_in, 16));
   CK(cudaMalloc(&d.out, 4096));
-  CK(cudaMalloc(&d.cyc, sizeof(long long) * d.n_sm * 8));
+  CK(cudaMalloc(&d.cyc, sizeof(long long) * d.n_sm * 16));
   std::printf("# warp-lane operations per clock per SM (slowest CTA), 8 independent chains/thread\n");
   std::printf("%-22s %8s %8s %8s\n", "instruction", "8 warps", "16 warps", "32 warps");
   single<FFMA_RRR>(d); single<FFMA_RRC>(d); single<FFMA_RIR>(d); single<FMUL_RR>(d);
@@ -243,5 +336,17 @@ int main() {
   mix<I2F_, MUFU_LG2>(d);
   mix<I2F_, LOP3_XOR3>(d);
   mix<I2F_, FFMA_RRR>(d);
+  std::printf("# the fp32 Euler-Maruyama step-loop mix as independent chains: SM cycles per warp and scheduler for\n"
+              "# one Philox block (four steps); the step kernel itself: kernel time x clock / (steps / 4) / warps per scheduler\n");
+  std::printf("%-44s %8s %8s %8s\n", "instructions per block", "4 CTA/SM", "9 CTA/SM", "12 CTA/SM");
+  loop_mix_row<1>(d, "54 FFMA/FMUL/FADD");
+  loop_mix_row<2>(d, "16 (IMAD.WIDE + LOP3)");
+  loop_mix_row<4>(d, "6 (FMUL.RZ + MUFU.COS) + 6 MUFU");
+  loop_mix_row<8>(d, "8 LOP3");
+  loop_mix_row<3>(d, "FP32 + Philox");
+  loop_mix_row<5>(d, "FP32 + MUFU");
+  loop_mix_row<6>(d, "Philox + MUFU");
+  loop_mix_row<7>(d, "FP32 + Philox + MUFU");
+  loop_mix_row<15>(d, "all (the step loop's mix, 118 instructions)");
   return 0;
 }
