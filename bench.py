@@ -40,6 +40,12 @@ N_SM, LANES_PER_SM = 148, 128
 # config[4] is bound by the FP64 pipe (64 lanes/clk/SM; 59 measured for DFMA), not by issue slots: its
 # I_alg counts the ~60 DFMA-pipe operations per particle-step and its peak is 64 lanes.
 LANES_FP64 = 64
+# dram__bytes_read.sum + dram__bytes_write.sum of the step kernel, per launch, from the committed
+# `ncu --set full` captures of the launch bench.py times (profiles/r01_step_kernel_cfg1_ncu_full.md,
+# profiles/r01_step_kernels_cfg2_cfg3_cfg4_ncu_full.md); None where no capture of that launch exists.
+# The frame (one, overwritten) and the state stay in the 126 MB L2 during a launch, so the traffic is
+# far BELOW the algorithmic bytes.
+NCU_TRAFFIC_BYTES = {1: 12_654_592}
 
 
 def load_peaks():
@@ -339,7 +345,8 @@ def run_ours(args, wl, cfg_id):
             "kernel_ms": 1e3 * t_k, "kernel_launches_per_pass": step_launches * (n_steps // M),
             "kernel_share_of_pass": sum(t_kern_ms) / sum(t_pass_ms),
             "peak_source": f"148 SMs x {lanes} lanes x sm_max_mhz {f_max / 1e6:.0f} MHz, {peak_src}",
-            "traffic": None,
+            "traffic": NCU_TRAFFIC_BYTES.get(cfg_id) if not args.sim_steps and args.rng == "philox" else None,
+            "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, committed capture)",
             "hbm_algorithmic_bytes_per_launch": int(T * (24 + 8 * (n_steps // wl.snapshot_every
                                                                    if wl.snapshot_every else 0))),
         }
