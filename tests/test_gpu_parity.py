@@ -708,3 +708,52 @@ def test_random_cases_against_the_oracle(abm, torch, oracle, case):
         om = oracle.moments(got[s][:, 0].copy(), got[s][:, 1].copy(), got[s][:, 2].copy(), x0f)
         for k_, val in om.items():
             assert m[k_][s] == pytest.approx(val, rel=1e-8, abs=1e-10), (case, s, k_)
+
+
+# ---------------------------------------------------------------------------------------------
+# abm_create of large sweeps: the coefficient table goes through the library's pinned staging buffer
+# (one per device, reused).  Two sweeps created back to back, and two created from two host threads
+# at once (one of them falls back to the malloc path), must both get their own coefficients.
+# ---------------------------------------------------------------------------------------------
+
+def _sweep_sets(q_scale, n_sets=8192):
+    wl = W.config2()
+    base = wl.set_params(0)
+    return [dict(base, D=1e-3 * (1 + s % 97), q=q_scale * (s % 251) / 250.0, F0=0.01 * (s % 13))
+            for s in range(n_sets)]
+
+
+def _check_sweep(oracle, sets, got, n_particles, seed, steps, picks):
+    for s in picks:
+        idx = np.arange(s * n_particles, (s + 1) * n_particles)
+        want = oracle_states(oracle, sets[s], seed, idx, steps)
+        err = scale_rel_err(got[idx], want)
+        assert np.all(err <= TOL_F32), (s, err)
+
+
+def test_large_sweeps_back_to_back_and_concurrent(abm, oracle):
+    import threading
+    n_particles, seed, steps = 4, 31, 40
+    sa, sb = _sweep_sets(1.0), _sweep_sets(2.0)
+    picks = [0, 1, 250, 4097, 8191]
+    # back to back on one stream: B's upload must not overwrite the table A's upload still reads
+    with abm.Ensemble(sa, n_particles, seed) as a, abm.Ensemble(sb, n_particles, seed) as b:
+        a.step(steps)
+        b.step(steps)
+        ga, gb = a.state(), b.state()
+    _check_sweep(oracle, sa, ga, n_particles, seed, steps, picks)
+    _check_sweep(oracle, sb, gb, n_particles, seed, steps, picks)
+    assert not np.array_equal(ga, gb)
+    # from two host threads at once
+    out = {}
+
+    def work(name, sets):
+        with abm.Ensemble(sets, n_particles, seed) as e:
+            e.step(steps)
+            out[name] = e.state()
+
+    for _ in range(3):
+        ts = [threading.Thread(target=work, args=("a", sa)), threading.Thread(target=work, args=("b", sb))]
+        [t.start() for t in ts]
+        [t.join() for t in ts]
+        assert np.array_equal(out["a"], ga) and np.array_equal(out["b"], gb)
