@@ -37,6 +37,9 @@
  *   - One context is not thread-safe; distinct contexts are independent.  All work of a context
  *     is enqueued on params[0].stream in call order; only abm_moments, abm_moment_sums,
  *     abm_snapshot_host and abm_destroy wait for it.
+ *   - A context belongs to the device that was current at abm_create.  Later calls may be made
+ *     with any device current: the library switches to the context's device and restores the
+ *     caller's before it returns.
  *   - There is no CPU fallback: without a CUDA device abm_create returns ABM_ECUDA.
  */
 #ifndef ABM_H

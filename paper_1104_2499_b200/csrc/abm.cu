@@ -438,6 +438,22 @@ int check_ctx(const abm_ctx* c) {
   return ABM_OK;
 }
 
+// Makes the context's device current for the duration of an API call and restores the caller's
+// device afterwards, so that a process driving several GPUs may call with any device current.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(const abm_ctx* c) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != c->device)
+      switched = cudaSetDevice(c->device) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 bool stride_ok(const abm_ctx* c, size_t stride) {
   return c->precision == ABM_FP32 ? (stride == 8 || stride == 16) : (stride == 16 || stride == 32);
 }
@@ -555,6 +571,7 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
 int abm_step(abm_ctx* c, uint64_t n_steps) {
   const int st = check_ctx(c);
   if (st != ABM_OK) return st;
+  const DeviceGuard on_device(c);
   if (n_steps == 0) return ABM_OK;
   return c->precision == ABM_FP32 ? step_impl<float>(c, n_steps) : step_impl<double>(c, n_steps);
 }
@@ -562,6 +579,7 @@ int abm_step(abm_ctx* c, uint64_t n_steps) {
 int abm_snapshot(abm_ctx* c, void* dev_ptr, size_t stride_bytes) {
   const int st = check_ctx(c);
   if (st != ABM_OK) return st;
+  const DeviceGuard on_device(c);
   if (!dev_ptr) {
     c->snap = nullptr;
     c->snap_stride = 0;
@@ -579,6 +597,7 @@ int abm_snapshot(abm_ctx* c, void* dev_ptr, size_t stride_bytes) {
 int abm_snapshot_host(abm_ctx* c, void* host_ptr, size_t stride_bytes) {
   const int st = check_ctx(c);
   if (st != ABM_OK) return st;
+  const DeviceGuard on_device(c);
   if (!host_ptr || !stride_ok(c, stride_bytes)) return ABM_EINVAL;
   const size_t bytes = stride_bytes * c->n_traj;
   if (c->frame_bytes < bytes) {
@@ -598,6 +617,7 @@ int abm_snapshot_host(abm_ctx* c, void* host_ptr, size_t stride_bytes) {
 int abm_moments(abm_ctx* c, abm_moment* out) {
   const int st = check_ctx(c);
   if (st != ABM_OK) return st;
+  const DeviceGuard on_device(c);
   if (!out) return ABM_EINVAL;
   const int rc = c->precision == ABM_FP32 ? reduce_moments<float>(c) : reduce_moments<double>(c);
   if (rc != ABM_OK) return rc;
@@ -610,6 +630,7 @@ int abm_moments(abm_ctx* c, abm_moment* out) {
 int abm_moment_sums(abm_ctx* c, double* out) {
   const int st = check_ctx(c);
   if (st != ABM_OK) return st;
+  const DeviceGuard on_device(c);
   if (!out) return ABM_EINVAL;
   const int rc = c->precision == ABM_FP32 ? reduce_moments<float>(c) : reduce_moments<double>(c);
   if (rc != ABM_OK) return rc;
@@ -623,6 +644,7 @@ int abm_raster(abm_ctx* c, uint32_t* dev_counts, uint32_t width, uint32_t height
                double v_max, uint8_t* dev_rgba, uint32_t saturation) {
   const int st = check_ctx(c);
   if (st != ABM_OK) return st;
+  const DeviceGuard on_device(c);
   if (!dev_counts || width == 0 || height == 0 || !(v_max > v_min) || !std::isfinite(v_min) ||
       !std::isfinite(v_max))
     return ABM_EINVAL;
@@ -712,8 +734,11 @@ int abm_get_accuracy(const abm_ctx* c, uint32_t* out_mode) {
 
 int abm_destroy(abm_ctx* c) {
   if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
-  cudaStreamSynchronize(c->stream);
-  free_all(c);
+  {
+    const DeviceGuard on_device(c);
+    cudaStreamSynchronize(c->stream);
+    free_all(c);
+  }
   c->magic = 0;
   delete c;
   return ABM_OK;
