@@ -89,6 +89,68 @@ def test_normals_consumed_by_the_step_kernel(abm, oracle):
             assert np.abs(z - want).mean() < 4e-7
 
 
+@pytest.mark.parametrize("traj_base", [0, 2**32 - 100], ids=["table", "straddle_2^32"])
+@pytest.mark.parametrize("K", [0, 4, 8, 100], ids=lambda k: f"K{k}")
+def test_normals_after_long_launches(abm, torch, oracle, K, traj_base):
+    """The same trick (v_{n+1} = sigma z_n exactly) over ONE long launch: the velocity after n steps is
+    the normal of step n - 1, whatever happened before.  Launch lengths are chosen around the refills
+    of the shared Philox block-head table (128 blocks = 512 steps), odd and even block counts (the
+    fp32 loop takes two blocks per trip), single-step tails, and frames every K steps (segments of
+    1, 2 and 25 blocks); traj_base = 2^32 - 100 puts the ensemble across a multiple of 2^32, where the
+    kernel runs without the table.  Pins the block <-> step <-> trajectory assignment of the fast path."""
+    dt = 2.0**-10
+    p = dict(W.DEFAULTS, A1=0.0, A2=0.0, d=0.0, q=0.0, c=0.0, gamma0=1.0 / dt, dt=dt, D=0.5 / dt)
+    N, seed = 300, 424242
+    done = 0
+    with abm.Ensemble([p], N, seed, snapshot_every=K, traj_base=traj_base) as ens:
+        frame = ens.bind_snapshot() if K else None
+        for n_launch in (512, 4, 1, 507, 1028, 2043, 5, 3000, 66000):
+            ens.step(n_launch)
+            done += n_launch
+            n = done - 1                                   # the step whose normal v now holds
+            z = ens.state()[:, 1]
+            pair = oracle.normals(seed, traj_base, N, n & ~1, 2, 0)
+            want, rho = pair[:, n & 1], np.hypot(pair[:, 0], pair[:, 1])
+            bound = 1.7e-7 / np.maximum(rho, 1e-4) + 1.0e-6 * (1.0 + rho)
+            assert np.all(np.abs(z - want) <= bound), (done, np.max(np.abs(z - want) / bound))
+            if K:                                          # the frame holds the last multiple of K
+                torch.cuda.synchronize()
+                m = (done // K) * K - 1
+                pf = oracle.normals(seed, traj_base, N, m & ~1, 2, 0)
+                wf, rf = pf[:, m & 1], np.hypot(pf[:, 0], pf[:, 1])
+                bf = 1.7e-7 / np.maximum(rf, 1e-4) + 1.0e-6 * (1.0 + rf)
+                assert np.all(np.abs(frame.cpu().numpy()[:, 1] - wf) <= bf), (done, m)
+
+
+@pytest.mark.parametrize("precision,rng", [(1, 0), (0, 1), (1, 1)], ids=["f64_philox", "f32_xorshift", "f64_xorshift"])
+def test_normals_after_long_launches_fp64_and_xorshift(abm, oracle, precision, rng):
+    """The same pin for the fp64 block loop (one block per trip) and for the xorshift fast path (its own
+    look-ahead loop), with a frame every 12 steps so that segments of three blocks alternate with tails."""
+    dt = 2.0**-10
+    p = dict(W.DEFAULTS, precision=precision, rng=rng, A1=0.0, A2=0.0, d=0.0, q=0.0, c=0.0,
+             gamma0=1.0 / dt, dt=dt, D=0.5 / dt)
+    N, seed, pick = 300, 77, slice(0, 300, 25)
+    done = 0
+    with abm.Ensemble([p], N, seed, snapshot_every=12) as ens:
+        ens.bind_snapshot()
+        for n_launch in (512, 4, 1, 507, 1028, 2043, 5):
+            ens.step(n_launch)
+            done += n_launch
+            n = done - 1
+            z = ens.state()[pick, 1]
+            if rng:
+                pair = np.array([[oracle.normal_xorshift(seed, k, n & ~1, precision),
+                                  oracle.normal_xorshift(seed, k, n | 1, precision)] for k in range(N)[pick]])
+            else:
+                pair = oracle.normals(seed, 0, N, n & ~1, 2, precision)[pick]
+            want, rho = pair[:, n & 1], np.hypot(pair[:, 0], pair[:, 1])
+            if precision:
+                bound = 1e-14 / np.maximum(rho, 1e-6) + 1e-14 * (1.0 + rho)
+            else:
+                bound = 1.7e-7 / np.maximum(rho, 1e-4) + 1.0e-6 * (1.0 + rho)
+            assert np.all(np.abs(z - want) <= bound), (done, np.max(np.abs(z - want) / bound))
+
+
 # ---------------------------------------------------------------------------------------------
 # per-trajectory state after 100 steps, small ensembles (several CTAs and a ragged tail)
 # ---------------------------------------------------------------------------------------------
