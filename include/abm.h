@@ -36,6 +36,7 @@
  *     snapshot buffer and all `out` arrays are caller-owned.
  *   - One context is not thread-safe; distinct contexts are independent.  All work of a context
  *     is enqueued on params[0].stream in call order; only abm_moments, abm_moment_sums,
+ *     abm_time_averaged_velocity,
  *     abm_snapshot_host and abm_destroy wait for it.
  *   - A context belongs to the device that was current at abm_create.  Later calls may be made
  *     with any device current: the library switches to the context's device and restores the
@@ -157,6 +158,13 @@ int abm_snapshot_host(abm_ctx* ctx, void* host_ptr, size_t stride_bytes);
 /* Ensemble moments of every set at the current step (S6): warp-shuffle + block + fixed-order
  * grid reduction in fp64 on the device, then a copy to out[0 .. n_param_sets) (HOST); waits. */
 int abm_moments(abm_ctx* ctx, abm_moment* out);
+
+/* The same reduction and copy, enqueued on the context's stream WITHOUT waiting: for moments every so
+ * many steps (BASELINE.json configs[3]) the integration then never stalls on a host round trip.
+ * out[0 .. n_param_sets) (HOST) must stay valid, and is defined, only after the stream has been
+ * synchronised by the caller (or by a later waiting call of this context); page-locked memory makes
+ * the copy a true asynchronous DMA, pageable memory is staged by the driver. */
+int abm_moments_async(abm_ctx* ctx, abm_moment* out);
 
 /* The raw sums (HOST, out[n_param_sets][ABM_N_SUMS]) and the pure host-side finalisation used
  * after summing shards: out_moments[s] from sums[s]. */

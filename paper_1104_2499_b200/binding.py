@@ -47,7 +47,7 @@ MOMENT_DTYPE = np.dtype([("n", "<u8"), ("step", "<u8"), ("mean_x", "<f8"), ("var
                          ("mean_v", "<f8"), ("var_v", "<f8"), ("mean_e", "<f8"),
                          ("mean_dx", "<f8"), ("mean_dx2", "<f8"), ("mean_x2", "<f8")])
 
-EXPORTS = ["abm_create", "abm_step", "abm_snapshot", "abm_snapshot_host", "abm_moments",
+EXPORTS = ["abm_create", "abm_step", "abm_snapshot", "abm_snapshot_host", "abm_moments", "abm_moments_async",
            "abm_moment_sums", "abm_moments_from_sums", "abm_time_averaged_velocity", "abm_raster", "abm_get_step", "abm_get_accuracy", "abm_destroy",
            "abm_philox_blocks", "abm_strerror", "abm_abi_version"]
 
@@ -75,6 +75,7 @@ def lib():
         L.abm_snapshot.argtypes = [vp, vp, C.c_size_t]
         L.abm_snapshot_host.argtypes = [vp, vp, C.c_size_t]
         L.abm_moments.argtypes = [vp, vp]
+        L.abm_moments_async.argtypes = [vp, vp]
         L.abm_moment_sums.argtypes = [vp, vp]
         L.abm_moments_from_sums.argtypes = [vp, u32, u64, vp]
         L.abm_time_averaged_velocity.argtypes = [vp, vp]
@@ -132,6 +133,14 @@ def abm_step(ctx, n_steps):
 
 def abm_snapshot(ctx, dev_ptr, stride_bytes):
     _check("abm_snapshot", lib().abm_snapshot(ctx, dev_ptr, stride_bytes))
+
+
+def abm_moments_async(ctx, n_param_sets, out):
+    """Enqueue the reduction and the copy into `out` (caller-owned record array [n_param_sets], pinned for a
+    true asynchronous copy) without waiting; `out` is defined once the caller has synchronised the stream."""
+    assert out.dtype == MOMENT_DTYPE and out.shape == (n_param_sets,) and out.flags.c_contiguous
+    _check("abm_moments_async", lib().abm_moments_async(ctx, out.ctypes.data))
+    return out
 
 
 def abm_snapshot_host(ctx, host_array, stride_bytes):
@@ -258,6 +267,9 @@ class Ensemble:
 
     def moments(self, out=None):
         return abm_moments(self.ctx, self.n_sets, out)
+
+    def moments_async(self, out):
+        return abm_moments_async(self.ctx, self.n_sets, out)
 
     def moment_sums(self, out=None):
         return abm_moment_sums(self.ctx, self.n_sets, out)

@@ -627,6 +627,18 @@ int abm_moments(abm_ctx* c, abm_moment* out) {
   return ABM_OK;
 }
 
+int abm_moments_async(abm_ctx* c, abm_moment* out) {
+  const int st = check_ctx(c);
+  if (st != ABM_OK) return st;
+  const DeviceGuard on_device(c);
+  if (!out) return ABM_EINVAL;
+  const int rc = c->precision == ABM_FP32 ? reduce_moments<float>(c) : reduce_moments<double>(c);
+  if (rc != ABM_OK) return rc;
+  ABM_CK(c, cudaMemcpyAsync(out, c->moments, sizeof(abm_moment) * c->n_sets,
+                            cudaMemcpyDeviceToHost, c->stream));
+  return ABM_OK;
+}
+
 int abm_moment_sums(abm_ctx* c, double* out) {
   const int st = check_ctx(c);
   if (st != ABM_OK) return st;
@@ -767,6 +779,6 @@ const char* abm_strerror(int status) {
   }
 }
 
-uint32_t abm_abi_version(void) { return 4; }
+uint32_t abm_abi_version(void) { return 5; }
 
 }  // extern "C"

@@ -34,7 +34,7 @@ def test_every_declared_symbol_is_exported(abm):
     L = abm.lib()
     for n in names:
         assert getattr(L, n) is not None
-    assert L.abm_abi_version() == 4
+    assert L.abm_abi_version() == 5
 
 
 def test_header_is_plain_c_and_layout_matches_ctypes(abm, tmp_path):
@@ -86,6 +86,7 @@ def test_error_paths_without_device(abm):
     assert L.abm_step(None, 1) == abm.ABM_ESTATE
     assert L.abm_destroy(None) == abm.ABM_ESTATE
     assert L.abm_moments(None, None) == abm.ABM_ESTATE
+    assert L.abm_moments_async(None, None) == abm.ABM_ESTATE
     assert L.abm_snapshot(None, None, 8) == abm.ABM_ESTATE
     assert L.abm_philox_blocks(1, 0, 0, 0, 1, None, None) == abm.ABM_EINVAL
     for code in (0, -1, -2, -3, -4, -99):

@@ -819,3 +819,22 @@ def test_large_sweeps_back_to_back_and_concurrent(abm, oracle):
         [t.start() for t in ts]
         [t.join() for t in ts]
         assert np.array_equal(out["a"], ga) and np.array_equal(out["b"], gb)
+
+
+def test_moments_async_matches_the_waiting_call(abm, torch):
+    """abm_moments_async enqueues reduction + copy without a host round trip; after the caller's stream
+    synchronisation every record equals, bit for bit, what abm_moments returns at the same step."""
+    wl = W.config3()
+    sets = [dict(wl.set_params(0), F0=0.1 * s) for s in range(3)]
+    n, seed = 1000, 5
+    slots = [abm.pinned_moment_buffers(len(sets))[0] for _ in range(4)]
+    with abm.Ensemble(sets, n, seed) as a, abm.Ensemble(sets, n, seed) as b:
+        for j in range(4):
+            a.step(50)
+            a.moments_async(slots[j][0])
+        torch.cuda.synchronize()
+        for j in range(4):
+            b.step(50)
+            m = b.moments()
+            assert int(m["step"][0]) == 50 * (j + 1)
+            assert np.array_equal(m.view(np.uint8), slots[j][0].view(np.uint8)), j
