@@ -41,6 +41,10 @@
  *   - A context belongs to the device that was current at abm_create.  Later calls may be made
  *     with any device current: the library switches to the context's device and restores the
  *     caller's before it returns.
+ *   - Small fp32 ensembles (up to 8,192 trajectories) are integrated by a kernel that splits the work
+ *     of a trajectory between warps (noise / integration) instead of one trajectory per thread; the
+ *     results are bit-identical.  The environment variable ABM_SMALL_MAX_TRAJ (read at abm_create)
+ *     moves that limit (0 = never): a tuning and test knob, not part of the semantics.
  *   - There is no CPU fallback: without a CUDA device abm_create returns ABM_ECUDA.
  */
 #ifndef ABM_H

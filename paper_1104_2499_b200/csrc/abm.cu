@@ -41,6 +41,7 @@ struct abm_ctx {
   bool precise;         // fp32 accuracy mode resolved at create (include/abm.h, abm_params.accuracy)
   uint64_t n_particles, n_traj, seed, step, traj_base, set_stride;
   double dt, omega;
+  uint64_t small_max_traj;  // ensembles up to this size run step_kernel_small (ABM_SMALL_MAX_TRAJ)
   double tilt_k0, tilt_A;  // what the tilt table holds: k0 + A cos(omega t) of the one set, or (0, 1)
   size_t real_size;
   void *x, *v, *e;      // state, SoA, Real[n_traj]
@@ -331,8 +332,26 @@ int upload_coefs_and_init(abm_ctx* c, const abm_params* params) {
   return ABM_OK;
 }
 
+// Ensembles of at most this many trajectories run the producer / consumer kernel (step_kernel_small):
+// below it the machine has more schedulers than the one-trajectory-per-thread kernel has warps.
+#ifndef ABM_SMALL_MAX_TRAJ
+#define ABM_SMALL_MAX_TRAJ 8192
+#endif
+
 template <typename Real, int INTEG, bool TILT, bool PRECISE, bool XS>
 cudaError_t launch_step_p(const abm_ctx* c, const StepArgs<Real>& a) {
+  if constexpr (sizeof(Real) == 4 && !XS) {
+    const bool frames_ok = a.snap == nullptr || a.snap_every == 0 || (a.snap_every & 3u) == 0;
+    if (c->n_traj <= c->small_max_traj && (a.step0 & 3u) == 0 && (a.n_steps & 3u) == 0 &&
+        a.n_steps >= 4 && frames_ok) {
+      const uint32_t g = static_cast<uint32_t>((c->n_traj + SMALL_TRAJ - 1) / SMALL_TRAJ);
+      if (c->n_sets == 1)
+        step_kernel_small<INTEG, TILT, true, PRECISE><<<g, SMALL_BLOCK, 0, c->stream>>>(a);
+      else
+        step_kernel_small<INTEG, TILT, false, PRECISE><<<g, SMALL_BLOCK, 0, c->stream>>>(a);
+      return cudaGetLastError();
+    }
+  }
   const uint32_t grid = static_cast<uint32_t>((c->n_traj + STEP_BLOCK - 1) / STEP_BLOCK);
   if (c->n_sets == 1)
     step_kernel<Real, INTEG, TILT, true, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
@@ -514,6 +533,12 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   c->tilt_k0 = n_param_sets == 1 ? (6.283185307179586476925286766559 / p0.L) * 2.0 * p0.A2 + p0.F0 : 0.0;
   c->tilt_A = n_param_sets == 1 ? p0.A : 1.0;
   c->real_size = c->precision == ABM_FP32 ? 4 : 8;
+  c->small_max_traj = ABM_SMALL_MAX_TRAJ;
+  if (const char* env = std::getenv("ABM_SMALL_MAX_TRAJ")) {  // tuning / test knob: results do not depend on it
+    char* end = nullptr;
+    const unsigned long long v = std::strtoull(env, &end, 10);
+    if (end != env) c->small_max_traj = v;
+  }
   c->precise = false;
   if (c->precision == ABM_FP32) {
     if (p0.accuracy == ABM_ACCURACY_PRECISE) c->precise = true;

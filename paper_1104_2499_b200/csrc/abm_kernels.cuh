@@ -180,6 +180,7 @@ struct Noise4<float> {
   Normal2f a, b;
   __device__ __forceinline__ Noise4(const uint4& w, const Coef<float>& k)
       : a(box_muller_f32(w.x, w.y, k.s2, k.bm_o)), b(box_muller_f32(w.z, w.w, k.s2, k.bm_o)) {}
+  __device__ __forceinline__ Noise4(const Normal2f& a_, const Normal2f& b_) : a(a_), b(b_) {}
 };
 template <>
 struct Noise4<double> {
@@ -203,11 +204,10 @@ __device__ __forceinline__ void one_step(State<Real>& s, const Coef<Real>& k, Re
   }
 }
 
-// Four steps from one Philox block.
+// Four steps from the noise of one Philox block.
 template <typename Real, int INTEG, int TILT, bool PRECISE>
-__device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf, const uint4& w,
-                                           const Real*& tl) {
-  const Noise4<Real> z(w, cf);
+__device__ __forceinline__ void four_steps_z(State<Real>& s, const Coef<Real>& cf,
+                                             const Noise4<Real>& z, const Real*& tl) {
   Real t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0;
   if (TILT) {
     t0 = tl[0]; t1 = tl[1]; t2 = tl[2]; t3 = tl[3];
@@ -220,6 +220,13 @@ __device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf,
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.cs, t2, t3);
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, rb, z.b.sn, t3, t4);
   if constexpr (PRECISE) fold(s, cf);  // after the step with global index 3 mod 4
+}
+// Four steps from one Philox block.
+template <typename Real, int INTEG, int TILT, bool PRECISE>
+__device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf, const uint4& w,
+                                           const Real*& tl) {
+  const Noise4<Real> z(w, cf);
+  four_steps_z<Real, INTEG, TILT, PRECISE>(s, cf, z, tl);
 }
 
 // The state as a frame shows it: in precise mode x is the remainder, the frame wants the position.
@@ -494,6 +501,103 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
     a.v[k] = s.v;
     a.e[k] = s.e;
     if (XS) a.rng_state[k] = S;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// The step kernel for SMALL ensembles (the paper's own regime: 2^0 ... 2^14 work items, PAPER.md:100,
+// where a launch is as slow as one warp's dependent chain, profiles/r01_scaling.md).  With fewer
+// warps than schedulers there is nothing to hide latency behind, so the work of one trajectory is
+// split between warps instead: a CTA is four warps around 32 trajectories -- warp 0 integrates
+// (force, update: the sequential part), warps 1-3 draw the noise of the coming Philox blocks
+// (Philox4x32-10 + Box-Muller: 60 % of the instructions, independent of the state) into a
+// double-buffered shared-memory ring of SMALL_CHUNK blocks; one __syncthreads per chunk.
+// The arithmetic is the same code as in step_kernel (four_steps_z on the same Noise4 values), so the
+// result is bit-identical to it -- trajectory i does not depend on which kernel ran.
+// fp32, Philox, launches made of whole Philox blocks with frames on block boundaries; everything
+// else goes to step_kernel.
+// ---------------------------------------------------------------------------------------------
+constexpr int SMALL_CHUNK = 16;    // Philox blocks per chunk (64 steps)
+constexpr int SMALL_TRAJ = 32;     // trajectories per CTA (one integrating warp)
+#ifndef ABM_SMALL_PRODUCERS
+#define ABM_SMALL_PRODUCERS 3
+#endif
+constexpr int SMALL_PRODUCERS = ABM_SMALL_PRODUCERS;            // noise warps per CTA
+constexpr int SMALL_BLOCK = 32 * (1 + SMALL_PRODUCERS);  // threads per CTA: 1 integrating warp + the noise warps
+
+template <int INTEG, bool TILT, bool UNIFORM, bool PRECISE>
+__global__ void __launch_bounds__(SMALL_BLOCK)
+step_kernel_small(const __grid_constant__ StepArgs<float> a) {
+  __shared__ float ring[2][SMALL_CHUNK][6][SMALL_TRAJ];
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;  // warp w issues from scheduler w
+  const uint64_t k_raw = static_cast<uint64_t>(blockIdx.x) * SMALL_TRAJ + lane;
+  const bool active = k_raw < a.n_traj;
+  const uint64_t k = active ? k_raw : a.n_traj - 1;  // idle lanes shadow the last trajectory
+  const TrajId id = traj_id(k, a.n_particles, a.traj_base, a.set_stride, UNIFORM);
+  const Coef<float> cf = UNIFORM ? a.coef0 : a.coef_table[id.set];
+  constexpr int TL = TILT ? (UNIFORM ? 2 : 1) : 0;
+
+  const uint32_t n_blocks = a.n_steps >> 2;         // the host sends whole blocks only
+  const uint64_t b0 = a.step0 >> 2;
+  const uint32_t n_chunks = (n_blocks + SMALL_CHUNK - 1) / SMALL_CHUNK;
+
+  auto produce = [&](uint32_t chunk, uint32_t buf) {  // warp w >= 1: blocks j = w - 1, w - 1 + SMALL_PRODUCERS, ...
+    const uint32_t first = chunk * SMALL_CHUNK;
+    const uint32_t cnt = n_blocks - first < SMALL_CHUNK ? n_blocks - first : SMALL_CHUNK;
+    for (uint32_t j = warp - 1u; j < cnt; j += SMALL_PRODUCERS) {
+      const Noise4<float> z(philox_block(a.seed, id.global, b0 + first + j), cf);
+      float(*slot)[SMALL_TRAJ] = ring[buf][j];
+      slot[0][lane] = z.a.rho; slot[1][lane] = z.a.cs; slot[2][lane] = z.a.sn;
+      slot[3][lane] = z.b.rho; slot[4][lane] = z.b.cs; slot[5][lane] = z.b.sn;
+    }
+  };
+
+  State<float> s{0.f, 0.f, 0.f, 0.f, 0u, 0, 0.f};
+  const float* tl = nullptr;
+  uint32_t to_snap = 0xffffffffu;  // blocks until the next frame (a launch has fewer than 2^30 steps)
+  const uint32_t K = a.snap != nullptr ? a.snap_every : 0u;
+  if (warp == 0) {
+    s.x = a.x[k]; s.v = a.v[k]; s.e = a.e[k];
+    if constexpr (PRECISE) {
+      s.xf = __float_as_uint(a.xl[k]);
+      s.xc = __float_as_int(a.xh[k]);
+      s.thb = fixed_angle(s.xf, cf.th_o);
+    }
+    if (TILT) tl = a.tilt + (a.step0 - a.tilt_base);
+    if (K) to_snap = static_cast<uint32_t>(((a.step0 / K + 1) * static_cast<uint64_t>(K) - a.step0) >> 2);
+  } else {
+    produce(0u, 0u);
+  }
+  __syncthreads();
+  uint32_t buf = 0;
+  for (uint32_t c = 0; c < n_chunks; ++c) {
+    if (warp == 0) {
+      const uint32_t first = c * SMALL_CHUNK;
+      const uint32_t cnt = n_blocks - first < SMALL_CHUNK ? n_blocks - first : SMALL_CHUNK;
+#pragma unroll 1
+      for (uint32_t j = 0; j < cnt; ++j) {
+        float(*slot)[SMALL_TRAJ] = ring[buf][j];
+        Normal2f za, zb;
+        za.rho = slot[0][lane]; za.cs = slot[1][lane]; za.sn = slot[2][lane];
+        zb.rho = slot[3][lane]; zb.cs = slot[4][lane]; zb.sn = slot[5][lane];
+        const Noise4<float> z(za, zb);
+        four_steps_z<float, INTEG, TL, PRECISE>(s, cf, z, tl);
+        if (--to_snap == 0) {
+          if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
+          to_snap = K >> 2;
+        }
+      }
+    } else if (c + 1 < n_chunks) {
+      produce(c + 1, buf ^ 1u);
+    }
+    __syncthreads();
+    buf ^= 1u;
+  }
+  if (warp == 0 && active) {
+    if constexpr (PRECISE) store_fixed(a.xl, a.xh, k, s.xf, s.xc);
+    a.x[k] = s.x;
+    a.v[k] = s.v;
+    a.e[k] = s.e;
   }
 }
 

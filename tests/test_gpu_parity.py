@@ -34,6 +34,19 @@ def torch():
     return torch
 
 
+@pytest.fixture(autouse=True, params=["auto", "one_per_thread"])
+def step_kernel_choice(request, monkeypatch):
+    """Every test runs twice: with the library's own choice between step_kernel_small (ensembles up to
+    8,192 trajectories, launches of whole Philox blocks) and step_kernel, and with step_kernel forced
+    (ABM_SMALL_MAX_TRAJ=0, read at abm_create) -- the small test ensembles would otherwise never reach
+    the kernel the full-size configs run."""
+    if request.param == "one_per_thread":
+        monkeypatch.setenv("ABM_SMALL_MAX_TRAJ", "0")
+    else:
+        monkeypatch.delenv("ABM_SMALL_MAX_TRAJ", raising=False)
+    return request.param
+
+
 def small(wl, n_particles, n_sets=None):
     """Same model and seed, fewer trajectories (sets are sub-sampled evenly)."""
     sets = range(wl.n_param_sets) if n_sets is None else \
@@ -838,3 +851,40 @@ def test_moments_async_matches_the_waiting_call(abm, torch):
             m = b.moments()
             assert int(m["step"][0]) == 50 * (j + 1)
             assert np.array_equal(m.view(np.uint8), slots[j][0].view(np.uint8)), j
+
+
+# ---------------------------------------------------------------------------------------------
+# step_kernel_small (noise warps + one integrating warp per 32 trajectories) against step_kernel
+# (one trajectory per thread): the same arithmetic, so the same bits -- state, frames and moments.
+# ---------------------------------------------------------------------------------------------
+
+BOTH_KERNELS = [
+    ("cfg0", W.config0, 4096, None, 0, 1000), ("cfg0_ragged", W.config0, 1000, None, 0, 264),
+    ("cfg0_8192", W.config0, 8192, None, 0, 64), ("cfg1_K100", W.config1, 700, None, 100, 1000),
+    ("cfg1_K8", W.config1, 33, None, 8, 200), ("cfg3", W.config3, 777, None, 0, 400),
+    ("cfg3_K4", W.config3, 100, None, 4, 64), ("cfg2_sets", W.config2, 64, 24, 0, 300),
+    ("cfg2_sets_K12", W.config2, 5, 100, 12, 120), ("one_trajectory", W.config0, 1, None, 4, 4000),
+]
+
+
+@pytest.mark.parametrize("name,mk,n,n_sets,K,steps", BOTH_KERNELS, ids=[c[0] for c in BOTH_KERNELS])
+def test_small_ensemble_kernel_is_bit_identical(abm, torch, monkeypatch, step_kernel_choice, name, mk, n, n_sets, K, steps):
+    if step_kernel_choice != "auto":
+        pytest.skip("compares both kernels itself")
+    wl = mk()
+    sets = small(wl, n, n_sets)
+    got = {}
+    for limit in ("0", "1000000"):
+        monkeypatch.setenv("ABM_SMALL_MAX_TRAJ", limit)
+        with abm.Ensemble(sets, n, wl.seed, snapshot_every=K) as ens:
+            frame = ens.bind_snapshot(with_e=True) if K else None
+            ens.step(steps // 2 // 4 * 4)           # two launches: the second starts from stored state
+            ens.step(steps - steps // 2 // 4 * 4)
+            st, m = ens.state(), ens.moments()
+            torch.cuda.synchronize()
+            got[limit] = (st, m.copy(), None if frame is None else frame.cpu().numpy())
+    a, b = got["0"], got["1000000"]
+    assert np.array_equal(a[0], b[0])
+    assert np.array_equal(a[1].view(np.uint8), b[1].view(np.uint8))
+    if K:
+        assert np.array_equal(a[2], b[2])
