@@ -417,8 +417,18 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
   a.traj_hi = static_cast<uint32_t>(g_first >> 32);
   a.traj_hi_shared = (g_first >> 32) == (g_last >> 32) ? 1u : 0u;
   const uint32_t chunk_max = c->tilt ? TILT_CHUNK : MAX_LAUNCH_STEPS;
+  // Small ensembles: step_kernel_small takes launches of whole Philox blocks that start on a block
+  // boundary, so a call is cut into [steps up to the boundary] [whole blocks] [rest]; split launches
+  // are bit-identical to one launch, whichever kernel runs them.
+  const bool small = sizeof(Real) == 4 && c->rng == ABM_RNG_PHILOX && c->n_traj <= c->small_max_traj &&
+                     (c->snap == nullptr || c->snap_every == 0 || (c->snap_every & 3u) == 0);
   while (n_steps > 0) {
-    const uint32_t chunk = static_cast<uint32_t>(n_steps < chunk_max ? n_steps : chunk_max);
+    uint32_t chunk = static_cast<uint32_t>(n_steps < chunk_max ? n_steps : chunk_max);
+    if (small) {
+      const uint32_t mis = static_cast<uint32_t>(c->step & 3u);
+      if (mis) chunk = chunk < 4u - mis ? chunk : 4u - mis;
+      else if (chunk >= 4u) chunk &= ~3u;
+    }
     a.step0 = c->step;
     a.tilt_base = c->step;
     a.n_steps = chunk;

@@ -864,6 +864,9 @@ BOTH_KERNELS = [
     ("cfg1_K8", W.config1, 33, None, 8, 200), ("cfg3", W.config3, 777, None, 0, 400),
     ("cfg3_K4", W.config3, 100, None, 4, 64), ("cfg2_sets", W.config2, 64, 24, 0, 300),
     ("cfg2_sets_K12", W.config2, 5, 100, 12, 120), ("one_trajectory", W.config0, 1, None, 4, 4000),
+    # "_odd": a one-step launch first, and step counts that are no multiple of 4 -- the library cuts each
+    # call into [steps to the block boundary] [whole blocks: step_kernel_small] [rest]
+    ("cfg0_odd", W.config0, 500, None, 0, 1003), ("cfg3_K8_odd", W.config3, 300, None, 8, 202),
 ]
 
 
@@ -878,6 +881,8 @@ def test_small_ensemble_kernel_is_bit_identical(abm, torch, monkeypatch, step_ke
         monkeypatch.setenv("ABM_SMALL_MAX_TRAJ", limit)
         with abm.Ensemble(sets, n, wl.seed, snapshot_every=K) as ens:
             frame = ens.bind_snapshot(with_e=True) if K else None
+            if name.endswith("_odd"):
+                ens.step(1)
             ens.step(steps // 2 // 4 * 4)           # two launches: the second starts from stored state
             ens.step(steps - steps // 2 // 4 * 4)
             st, m = ens.state(), ens.moments()
