@@ -339,7 +339,9 @@ def run_ours(args, wl, cfg_id):
         achieved = lane_instr / t_k
         sm_mhz = clocks.get("sm_mhz") or (f_max / 1e6)
         out["roofline"] = {
-            "bound": "alu", "kernel": "abm::step_kernel", "achieved": achieved / 1e12,
+            "bound": "alu",
+            "kernel": "abm::step_kernel_small" if (not fp64 and args.rng == "philox" and T <= 8192) else "abm::step_kernel",
+            "achieved": achieved / 1e12,
             "peak": peak / 1e12,
             "unit": "Tinstr/s (FP64-pipe lane operations)" if fp64 else "Tinstr/s (warp-lane instructions)",
             "frac": achieved / peak,
