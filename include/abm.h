@@ -131,9 +131,9 @@ typedef struct abm_moment {
 } abm_moment; /* 80 bytes */
 
 /* Raw fp64 sums behind abm_moment, for combining shards (one record per set):
- * s = { N, sum x, sum x^2, sum v, sum v^2, sum e, sum dx, sum dx^2 },
- * with x and v taken relative to the set's first trajectory's initial values is NOT done:
- * the sums are plain; they are accumulated in fp64 in a fixed order (run-to-run reproducible). */
+ * s = { N, sum x, sum x^2, sum v, sum v^2, sum e, sum dx, sum dx^2 }
+ * -- plain sums (no shift of origin), accumulated in fp64 in a fixed order (run-to-run
+ * reproducible). */
 #define ABM_N_SUMS 8
 
 /* Create a context for n_param_sets parameter sets x n_particles trajectories each and
