@@ -143,3 +143,47 @@ def test_product_never_imports_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(import|from)\s+paper_1104_2499_b200", txt, flags=re.M)
             assert '#include "abm.h"' not in txt and "abm_device" not in txt
+
+
+def _build_c_demo(tmp_path):
+    exe = tmp_path / "abm_demo"
+    pkg = os.path.join(ROOT, "paper_1104_2499_b200")
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-o", str(exe),
+                    os.path.join(pkg, "examples", "abm_demo.c"), "-L", pkg, "-labm_b200",
+                    "-Wl,-rpath," + pkg], check=True)
+    return exe
+
+
+def test_plain_c_caller_links_and_fails_loudly_without_a_device(abm, tmp_path):
+    """The boundary is a C library: a C99 program with no CUDA headers links against it.  Without a
+    device it must report ABM_ECUDA (exit code 3 of the demo), never compute on the CPU."""
+    import torch
+    exe = _build_c_demo(tmp_path)
+    r = subprocess.run([str(exe), "8", "4"], capture_output=True, text=True)
+    if torch.cuda.is_available():
+        assert r.returncode == 0, r.stderr
+    else:
+        assert r.returncode == 3 and "abm_create: -3" in r.stderr, (r.returncode, r.stderr)
+
+
+@pytest.mark.gpu
+def test_plain_c_caller_matches_the_oracle(abm, tmp_path):
+    """The same program on the GPU box: its printed state and moments against the CPU oracle."""
+    import numpy as np
+    from paper_1104_2499_b200 import workloads as W
+    from oracle import abm_oracle as orc
+    exe = _build_c_demo(tmp_path)
+    n, steps = 300, 100
+    r = subprocess.run([str(exe), str(n), str(steps)], capture_output=True, text=True, check=True)
+    lines = r.stdout.strip().splitlines()
+    got = np.array([[float(t) for t in ln.split()[2:5]] for ln in lines[1:]])
+    assert got.shape == (n, 3)
+    p = W.config0().set_params(0)
+    x, v, e = orc.init_many(p, 42, n)
+    orc.run(p, 42, x, v, e, 0, steps)
+    want = np.stack([x, v, e], 1)
+    rms = np.sqrt((want**2).mean(0))
+    assert np.all(np.abs(got - want) / np.maximum(np.abs(want), rms) <= 1e-5)
+    mom = dict(zip(lines[0].split()[1::2], lines[0].split()[2::2]))
+    assert int(mom["n"]) == n and int(mom["step"]) == steps
+    assert abs(float(mom["mean_v"]) - got[:, 1].mean()) <= 1e-6
