@@ -893,3 +893,30 @@ def test_small_ensemble_kernel_is_bit_identical(abm, torch, monkeypatch, step_ke
     assert np.array_equal(a[1].view(np.uint8), b[1].view(np.uint8))
     if K:
         assert np.array_equal(a[2], b[2])
+
+
+def test_more_than_2_to_31_trajectories(abm, torch, oracle, step_kernel_choice):
+    """Maximum-size edge: 2^31 + 4097 trajectories in one context (26 GB of state, a 17 GB frame) -- every
+    index in the kernels is 64-bit.  Sampled trajectories on both sides of 2^31 and at the ragged end
+    against the oracle; the count and the mean of the uniform initial positions from the reduction."""
+    if step_kernel_choice != "auto":
+        pytest.skip("one kernel choice is enough for this size")
+    free, _total = torch.cuda.mem_get_info()
+    if free < 60 * 2**30:
+        pytest.skip("needs 60 GB of free device memory")
+    wl = W.config0()
+    p = wl.set_params(0)
+    N, steps = 2**31 + 4097, 8
+    with abm.Ensemble([p], N, wl.seed, snapshot_every=4) as ens:
+        frame = ens.bind_snapshot()
+        m0 = ens.moments()[0]
+        ens.step(steps)
+        m = ens.moments()[0]
+        idx = np.array([0, 1, 127, 128, 2**31 - 129, 2**31 - 1, 2**31, 2**31 + 1, 2**31 + 4095, N - 2, N - 1])
+        got = frame[torch.as_tensor(idx, device=frame.device)].cpu().numpy().astype(np.float64)
+    assert int(m0["n"]) == N == int(m["n"]) and int(m["step"]) == steps
+    assert abs(float(m0["mean_x"]) - 0.5) < 1e-4 and abs(float(m0["var_x"]) - 1.0 / 12.0) < 1e-4
+    want = oracle_states(oracle, p, wl.seed, idx, steps)[:, :2]
+    assert np.all(np.abs(got - want) <= 1e-6 * np.maximum(1.0, np.abs(want))), np.abs(got - want).max()
+    del frame
+    torch.cuda.empty_cache()
