@@ -45,7 +45,9 @@ LANES_FP64 = 64
 # profiles/r01_step_kernels_cfg2_cfg3_cfg4_ncu_full.md); None where no capture of that launch exists.
 # The frame (one, overwritten) and the state stay in the 126 MB L2 during a launch, so the traffic is
 # far BELOW the algorithmic bytes.
-NCU_TRAFFIC_BYTES = {1: 12_654_592}
+# configs[2-4] were captured on launches shortened with --sim-steps; a launch reads the state once and
+# writes it once whatever its step count (config[3]: 1,000 steps per launch in both), so the figure holds.
+NCU_TRAFFIC_BYTES = {1: 12_654_592, 2: 55_608_832 + 825_088, 3: 21_009_664, 4: 101_598_464 + 42_590_976}
 
 
 def load_peaks():
