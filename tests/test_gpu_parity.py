@@ -730,7 +730,7 @@ def test_tilt_table_across_launch_chunks(abm):
 # randomised differential test: random (seeded) models, sizes, launch splits and frame periods
 # ---------------------------------------------------------------------------------------------
 
-@pytest.mark.parametrize("case", range(24))
+@pytest.mark.parametrize("case", range(64))
 def test_random_cases_against_the_oracle(abm, torch, oracle, case):
     rng = np.random.default_rng(9000 + case)
     precision = int(rng.integers(0, 2))
@@ -768,6 +768,11 @@ def test_random_cases_against_the_oracle(abm, torch, oracle, case):
         assert np.array_equal(got, ref.state())                       # independent of splits and of frames
     got = got.reshape(n_sets, n, 3)
     tol = (TOL_F32 if precision == 0 else TOL_F64) * max(1.0, total / 100.0)
+    if precision == 0 and acc == abm.ABM_ACCURACY_FAST:
+        # FAST forced on a set AUTO would run in PRECISE mode (the fp32 deviation grows with
+        # dt max|U''|; AUTO switches above 0.15): the bound is scaled by how far beyond that the set is
+        stiff = max(p["dt"] * (2 * math.pi / p["L"])**2 * (abs(p["A1"]) + 4 * abs(p["A2"])) for p in sets)
+        tol *= max(1.0, stiff / 0.15)
     for s, p in enumerate(sets):
         first = base_idx + s * n
         x, v, e = oracle.init_many(p, seed, n, first)
