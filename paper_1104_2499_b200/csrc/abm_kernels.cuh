@@ -310,11 +310,26 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
           const uint32_t seg = left < to_snap ? left : static_cast<uint32_t>(to_snap);  // >= 1
           const bool last = seg == left;
           uint32_t ahead = last ? seg - 1u : seg;  // blocks of this segment with a look-ahead draw
+          if constexpr (sizeof(Real) == 4 && ABM_UNROLL2 != 0) {  // two blocks per trip, as for Philox
+            if (ahead & 1u) {
+              const uint4 w_next = xorshift128_x4(S);
+              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+              w = w_next;
+            }
 #pragma unroll 1
-          for (; ahead; --ahead) {
-            const uint4 w_next = xorshift128_x4(S);
-            four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
-            w = w_next;
+            for (ahead >>= 1; ahead; --ahead) {
+              const uint4 wa = xorshift128_x4(S);
+              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+              w = xorshift128_x4(S);
+              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, wa, tl);
+            }
+          } else {
+#pragma unroll 1
+            for (; ahead; --ahead) {
+              const uint4 w_next = xorshift128_x4(S);
+              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+              w = w_next;
+            }
           }
           if (last) four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
           left -= seg;
