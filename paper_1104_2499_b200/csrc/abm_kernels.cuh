@@ -15,7 +15,8 @@ namespace abm {
 // moves -- not for latency hiding.
 // Measured on B200 (round-1 sweeps, particle-steps/s): fp32 EM one set 8 > 7 > 5 > 6 > 12;
 // fp32 Heun 5 ~ 4 > 6 > 8; fp32 with per-thread coefficients 4 > 6 > 8 > 12 (12 spilled 236 B);
-// fp64 insensitive between 4 and 8 (12 spilled > 1 KB).
+// fp64 (final loop of the round, 2,000 steps of config[4]): 5: 27.51 ms ~ 4: 27.63 < 3: 28.17 < 7: 28.28
+// < 6: 28.54 < 8: 28.75 (16 B of stack per thread in the loop); 12 spilled > 1 KB.
 #ifndef ABM_MINB_F32U
 #define ABM_MINB_F32U 8   // fp32 Euler-Maruyama, one parameter set (uniform coefficients): <= 64 regs
 #endif
@@ -26,7 +27,7 @@ namespace abm {
 #define ABM_MINB_F32N 4   // fp32, per-thread coefficient record (config[2]): <= 128 regs
 #endif
 #ifndef ABM_MINB_F64
-#define ABM_MINB_F64 8    // fp64: <= 64 regs
+#define ABM_MINB_F64 5    // fp64: <= 96 regs (ptxas takes 86: no stack traffic in the loop)
 #endif
 constexpr int STEP_BLOCK = ABM_STEP_BLOCK;   // threads per CTA of the step kernel
 template <typename Real, int INTEG, bool UNIFORM>
