@@ -13,12 +13,13 @@ namespace abm {
 // (profiles/r01_scaling.md: no wave quantisation, a partly filled wave runs proportionally
 // faster), so occupancy is chosen for the code ptxas produces under the cap -- no spills, few
 // moves -- not for latency hiding.
-// Measured on B200 (round-1 sweeps, particle-steps/s): fp32 EM one set 8 > 7 > 5 > 6 > 12;
+// Measured on B200 (round-1 sweeps, particle-steps/s): fp32 EM one set, final loop of the round (20,000 steps of
+// config[1]): 5: 22.32 ms < 3 ~ 4: 22.47 < 6 ~ 8: 22.50 < 7 ~ 10: 22.91 < 12: 23.22;
 // fp32 Heun 5 ~ 4 > 6 > 8; fp32 with per-thread coefficients 4 > 6 > 8 > 12 (12 spilled 236 B);
 // fp64 (final loop of the round, 2,000 steps of config[4]): 5: 27.51 ms ~ 4: 27.63 < 3: 28.17 < 7: 28.28
 // < 6: 28.54 < 8: 28.75 (16 B of stack per thread in the loop); 12 spilled > 1 KB.
 #ifndef ABM_MINB_F32U
-#define ABM_MINB_F32U 8   // fp32 Euler-Maruyama, one parameter set (uniform coefficients): <= 64 regs
+#define ABM_MINB_F32U 5   // fp32 Euler-Maruyama, one parameter set (uniform coefficients): <= 96 regs (ptxas takes 62)
 #endif
 #ifndef ABM_MINB_F32H
 #define ABM_MINB_F32H 5   // fp32 Heun, one parameter set: <= 96 regs
