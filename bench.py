@@ -47,7 +47,7 @@ LANES_FP64 = 64
 # far BELOW the algorithmic bytes.
 # configs[2-4] were captured on launches shortened with --sim-steps; a launch reads the state once and
 # writes it once whatever its step count (config[3]: 1,000 steps per launch in both), so the figure holds.
-NCU_TRAFFIC_BYTES = {1: 12_654_592, 2: 55_608_832 + 825_088, 3: 21_009_664, 4: 101_443_328 + 46_812_416}
+NCU_TRAFFIC_BYTES = {1: 12_684_800, 2: 55_608_832 + 825_088, 3: 21_009_664, 4: 101_443_328 + 46_812_416}
 
 
 def load_peaks():
