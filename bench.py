@@ -11,9 +11,18 @@ stream, parameters already marshalled); `e2e` times the same pass by wall clock 
 C ABI from HOST parameter records to HOST results, including a device->host copy of the final
 frame into pinned memory and of the moments.
 
-N > 1 (torchrun): each rank integrates its own shard of a N-times larger ensemble (weak scaling;
-trajectory indices rank*T ... via traj_base), and the only exchange is one all-reduce of the
-per-set raw moment sums (8 doubles per set) over NCCL, inside the timed region.
+N > 1: one process per GPU.  Under torchrun (WORLD_SIZE set) this process is one rank; a bare
+`python bench.py --gpus N` re-executes itself under `python -m torch.distributed.run --nproc-per-node N`
+(127.0.0.1 rendezvous) and fails loudly if the box has fewer than N devices.  Each rank integrates its
+own shard of a N-times larger ensemble (weak scaling; trajectory indices rank*T ... via traj_base), and
+the only exchange is one all-reduce of the per-set raw moment sums (8 doubles per set) over NCCL on the
+device (sharding.MomentExchange: no host round trip), inside the timed region.
+
+Timing protocol of the paper (PAPER.md:100 "20 steps ... last fifteen", :122 "average and standard
+deviation ... zero steps ... offset time"): besides the mean, the line carries the standard deviation over
+the timed passes (`ms_per_step_sd`, `roofline.kernel_ms_sd`) and `offset_ms`: 20 launches of ONE step on the
+same ensemble, the last 15 averaged -- what a launch costs before any iteration is done (load + store of the
+state, launch latency).
 
 --impl reference times the CPU oracle (oracle/, plain fp64 C) on a bounded sample of the same
 workload on the host cores: a deliberately slow program, reported as the baseline, not the target.
@@ -41,13 +50,34 @@ N_SM, LANES_PER_SM = 148, 128
 # I_alg counts the ~60 DFMA-pipe operations per particle-step and its peak is 64 lanes.
 LANES_FP64 = 64
 # dram__bytes_read.sum + dram__bytes_write.sum of the step kernel, per launch, from the committed
-# `ncu --set full` captures of the launch bench.py times (profiles/r01_step_kernel_cfg1_ncu_full.md,
-# profiles/r01_step_kernels_cfg2_cfg3_cfg4_ncu_full.md); None where no capture of that launch exists.
+# `ncu --set full` captures of the launch bench.py times (profiles/*_ncu_full.md), each with the git blob
+# ids of the two kernel sources it was captured on: when a source has changed since, the figure is stale
+# and the line says `"traffic": null` instead (re-capture, then update the entry).
 # The frame (one, overwritten) and the state stay in the 126 MB L2 during a launch, so the traffic is
-# far BELOW the algorithmic bytes.
-# configs[2-4] were captured on launches shortened with --sim-steps; a launch reads the state once and
-# writes it once whatever its step count (config[3]: 1,000 steps per launch in both), so the figure holds.
-NCU_TRAFFIC_BYTES = {1: 12_684_800, 2: 55_608_832 + 825_088, 3: 21_009_664, 4: 101_443_328 + 46_812_416}
+# far BELOW the algorithmic bytes.  configs[2-4] were captured on launches shortened with --sim-steps; a
+# launch reads the state once and writes it once whatever its step count, so the figure holds.
+NCU_TRAFFIC = {
+    # cfg: (bytes per launch, blob of csrc/abm_kernels.cuh, blob of csrc/abm_device.cuh, summary)
+}
+# Warp-lane instructions per particle-step of the xorshift variant are not frozen anywhere: no `frac` for it.
+
+
+def git_blob(path):
+    """What `git hash-object` prints for the file."""
+    import hashlib
+    data = open(path, "rb").read()
+    return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
+
+
+def ncu_traffic(cfg_id):
+    ent = NCU_TRAFFIC.get(cfg_id)
+    if not ent:
+        return None, "no committed capture of this launch"
+    csrc = os.path.join(ROOT, "paper_1104_2499_b200", "csrc")
+    now = (git_blob(os.path.join(csrc, "abm_kernels.cuh")), git_blob(os.path.join(csrc, "abm_device.cuh")))
+    if now != (ent[1], ent[2]):
+        return None, f"stale: kernel sources changed since the capture in {ent[3]}"
+    return ent[0], f"ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, {ent[3]}"
 
 
 def load_peaks():
@@ -197,15 +227,23 @@ def run_ours(args, wl, cfg_id):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference "
                          "for the oracle)")
-    torch.cuda.set_device(local_rank % torch.cuda.device_count())
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE is {world}: launch one rank per GPU "
+                         f"(torchrun --nproc-per-node {args.gpus}, or the bare `python bench.py --gpus N`)")
+    n_dev = torch.cuda.device_count()
+    if args.backend == "nccl" and n_dev < world:
+        raise SystemExit(f"bench.py: --gpus {world} needs {world} CUDA devices, this box has {n_dev} "
+                         "(--backend gloo rehearses the multi-rank flow with ranks sharing a GPU)")
+    torch.cuda.set_device(local_rank % n_dev)
     if world > 1:
         if args.backend == "nccl":
             dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         else:   # gloo: exercises the multi-rank flow where ranks must share one GPU (NCCL refuses that)
             dist.init_process_group("gloo")
     coll_dev = "cuda" if args.backend == "nccl" else "cpu"
-    if world > 1 and args.backend != "nccl":
-        torch.cuda.set_device(local_rank % torch.cuda.device_count())
+    print(f"[bench rank {rank}/{world}] cuda:{torch.cuda.current_device()} "
+          f"{torch.cuda.get_device_name()} backend {args.backend if world > 1 else 'none'}",
+          file=sys.stderr, flush=True)
     abm.lib()
 
     stream = torch.cuda.Stream()
@@ -224,6 +262,8 @@ def run_ours(args, wl, cfg_id):
     (mom_out, _mom_keep), (sums_out, _sums_keep) = abm.pinned_moment_buffers(len(sets))  # pinned: true DMA
     # one pinned record array per intermediate reduction of a pass (config[3]: 19)
     mom_slots = [abm.pinned_moment_buffers(len(sets))[0] for _ in range(max(n_steps // M - 1, 0))]
+    # N > 1: device + pinned buffers of the one exchange, a slot per reduction of a pass
+    exchange = sharding.MomentExchange(plan, n_slots=n_steps // M, backend=args.backend) if world > 1 else None
     launches = {"n": 0}
     ens_tilt = any(p["A"] != 0.0 for p in sets)
     step_launches = (2 if ens_tilt else 1) * -(-M // (65536 if ens_tilt else 2**30))
@@ -248,8 +288,8 @@ def run_ours(args, wl, cfg_id):
                 if ev is not None:
                     ev[j][1].record(stream)
                 launches["n"] += step_launches
-                if world > 1:                                                  # S6 (2 kernels) + NCCL
-                    m = sharding.reduce_moments(ens.moment_sums(sums_out), ens.step_count, plan, device=coll_dev)
+                if world > 1:                          # S6 (2 kernels) + all-reduce, enqueued: no host round trip
+                    exchange.enqueue(ens, j)
                 elif j + 1 < n_steps // M:     # intermediate reductions: enqueued, no host round trip
                     ens.moments_async(mom_slots[j][0])                         # S6 (2 kernels)
                 else:                          # the last one waits: every record is on the host now
@@ -258,7 +298,9 @@ def run_ours(args, wl, cfg_id):
             if e2e:
                 abm.abm_snapshot_host(ens.ctx, host_frame.numpy(), frame_cols * frame_item)
                 launches["n"] += 1
-            ens.close()
+            ens.close()                                # waits for the stream: every record is on the host
+            if world > 1:
+                m = exchange.result(n_steps // M - 1)
         return m
 
     def barrier():
@@ -301,6 +343,20 @@ def run_ours(args, wl, cfg_id):
     barrier()
     t_e2e = time.perf_counter() - t0
 
+    # ---- the paper's "offset time": 20 launches of one step, the last 15 ----
+    with torch.cuda.stream(stream):
+        ens = abm.Ensemble(params, wl.n_particles, wl.seed, stream=stream)
+        if wl.snapshot_every:
+            ens.bind_snapshot()
+        ev_off = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+        for a, b in ev_off:
+            a.record(stream)
+            ens.step(1)
+            b.record(stream)
+        stream.synchronize()
+        ens.close()
+    t_off = [a.elapsed_time(b) for a, b in ev_off][5:]
+
     tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=coll_dev)
     if world > 1:
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
@@ -316,6 +372,9 @@ def run_ours(args, wl, cfg_id):
         "metric": "particle-steps/sec", "value": value, "unit": "particle-steps/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak",
+        "ms_per_step_sd": statistics.pstdev(t_pass_ms) if len(t_pass_ms) > 1 else None,   # this rank's passes
+        "offset_ms": {"mean": statistics.mean(t_off), "sd": statistics.pstdev(t_off),
+                      "protocol": "20 launches of 1 step, last 15 (PAPER.md:100, :122)"},
         "vs_baseline": None,   # the paper states no throughput for this path
         "dtype": "f64" if fp64 else "f32", "data": "synthetic",
         "config": {"workload": wl.name, "baseline_config": cfg_id, "trajectories_per_gpu": T,
@@ -340,21 +399,24 @@ def run_ours(args, wl, cfg_id):
         peak = N_SM * lanes * f_max
         achieved = lane_instr / t_k
         sm_mhz = clocks.get("sm_mhz") or (f_max / 1e6)
+        traffic, traffic_src = ncu_traffic(cfg_id) if (not args.sim_steps and args.rng == "philox") else \
+            (None, "no capture of this launch (--sim-steps / --rng xorshift)")
+        philox = args.rng == "philox"
         out["roofline"] = {
             "bound": "alu",
             "kernel": "abm::step_kernel_small" if (not fp64 and args.rng == "philox" and T <= 8192) else "abm::step_kernel",
-            "achieved": achieved / 1e12,
+            "achieved": achieved / 1e12 if philox else None,
             "peak": peak / 1e12,
             "unit": "Tinstr/s (FP64-pipe lane operations)" if fp64 else "Tinstr/s (warp-lane instructions)",
-            "frac": achieved / peak,
-            "frac_at_sustained_clock": achieved / (N_SM * lanes * sm_mhz * 1e6),
-            "i_alg_per_particle_step": I_ALG[cfg_id],
+            "frac": achieved / peak if philox else None,     # I_alg is frozen for the Philox path only
+            "frac_at_sustained_clock": achieved / (N_SM * lanes * sm_mhz * 1e6) if philox else None,
+            "i_alg_per_particle_step": I_ALG[cfg_id] if philox else None,
             "particle_steps_per_pass": wl.particle_steps,
-            "kernel_ms": 1e3 * t_k, "kernel_launches_per_pass": step_launches * (n_steps // M),
+            "kernel_ms": 1e3 * t_k, "kernel_ms_sd": statistics.pstdev(t_kern_ms) if len(t_kern_ms) > 1 else None,
+            "kernel_launches_per_pass": step_launches * (n_steps // M),
             "kernel_share_of_pass": sum(t_kern_ms) / sum(t_pass_ms),
             "peak_source": f"148 SMs x {lanes} lanes x sm_max_mhz {f_max / 1e6:.0f} MHz, {peak_src}",
-            "traffic": NCU_TRAFFIC_BYTES.get(cfg_id) if not args.sim_steps and args.rng == "philox" else None,
-            "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum, committed capture)",
+            "traffic": traffic, "traffic_source": traffic_src,
             "hbm_algorithmic_bytes_per_launch": int(T * (24 + 8 * (n_steps // wl.snapshot_every
                                                                    if wl.snapshot_every else 0))),
         }
@@ -367,6 +429,17 @@ def run_ours(args, wl, cfg_id):
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def launcher_command(argv, n_gpus, port=None):
+    """The command a bare `python bench.py --gpus N` (N > 1, no WORLD_SIZE) re-executes: one rank per GPU."""
+    if port is None:
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}",
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
 
 
 def main():
@@ -390,8 +463,16 @@ def main():
             wl.moments_every = min(wl.moments_every, wl.n_steps)
     if args.impl == "reference":
         run_reference(args, wl)
-    else:
-        run_ours(args, wl, args.config)
+        return
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under torchrun: start the N ranks ourselves (one process per GPU)
+        import subprocess
+        cmd = launcher_command(sys.argv[1:], args.gpus)
+        print("bench.py: launching " + " ".join(cmd), file=sys.stderr, flush=True)
+        raise SystemExit(subprocess.call(cmd))
+    run_ours(args, wl, args.config)
 
 
 if __name__ == "__main__":

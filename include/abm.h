@@ -32,8 +32,9 @@
  *     whole trajectory, depends only on (seed, i, parameters): shards of one ensemble on
  *     several GPUs use traj_base / traj_set_stride to address disjoint index ranges.
  *   - In device buffers trajectories are stored in local order  k = set * n_particles + r.
- *   - The library owns the state and its scratch; `params` may be freed after abm_create; the
- *     snapshot buffer and all `out` arrays are caller-owned.
+ *   - The library owns the state and its scratch (device memory from a library-owned stream-ordered
+ *     pool that keeps at most 1 GiB of freed memory cached; abm_trim releases it); `params` may be
+ *     freed after abm_create; the snapshot buffer and all `out` arrays are caller-owned.
  *   - One context is not thread-safe; distinct contexts are independent.  All work of a context
  *     is enqueued on params[0].stream in call order; only abm_moments, abm_moment_sums,
  *     abm_time_averaged_velocity,
@@ -43,8 +44,11 @@
  *     caller's before it returns.
  *   - Small fp32 ensembles (up to 8,192 trajectories) are integrated by a kernel that splits the work
  *     of a trajectory between warps (noise / integration) instead of one trajectory per thread; the
- *     results are bit-identical.  The environment variable ABM_SMALL_MAX_TRAJ (read at abm_create)
- *     moves that limit (0 = never): a tuning and test knob, not part of the semantics.
+ *     results are bit-identical.  abm_params.step_kernel overrides the choice: a tuning and test knob,
+ *     not part of the semantics.  The library reads no environment variable.
+ *   - A handle is valid from a successful abm_create until abm_destroy.  Calls on a NULL, never
+ *     created or already destroyed handle return ABM_ESTATE (handles are looked up in a table of live
+ *     contexts before they are dereferenced; as with any address, a NEW context may later reuse it).
  *   - There is no CPU fallback: without a CUDA device abm_create returns ABM_ECUDA.
  */
 #ifndef ABM_H
@@ -78,11 +82,24 @@ enum { ABM_INIT_V_CONST = 0, ABM_INIT_V_THERMAL = 1 }; /* abm_params.init_v */
  *            most four steps, so nothing is rounded at the magnitude of the unwrapped position;
  *            the force takes its angle from the fraction word.  About +1.5 instructions per step
  *            over FAST, two more words of state per trajectory.  Frames, moments and the raster see
- *            the position rounded once to fp32.  Needs 4 |v| dt < L / 2.
+ *            the position rounded once to fp32.  The offset is folded with a 64-bit conversion, so
+ *            any speed is legal (|x| < 2^31 L).
  *   AUTO     PRECISE if dt (2 pi / L)^2 (|A1| + 4 |A2|) > 0.15 for any set, else FAST
  *            (configs[0-2]: 0.079 -> FAST; config[3]: 0.39 -> PRECISE).
+ * What the modes promise.  S = dt max|U''| <= dt (2 pi / L)^2 (|A1| + 4 |A2|) is the factor by which one
+ * step turns a position error into a velocity error; the 100-step deviation from the fp64 oracle grows
+ * in proportion to it.  FAST holds 1e-5 (scale-relative, reading G14) for S <= 0.15; forced on
+ * a stiffer set it may miss it by about S / 0.15.  PRECISE holds 1e-5 for S <= 0.3 (config[3]: 0.39 is
+ * measured at 4.4e-6, but random stiff potentials at 0.39 and 0.53 have missed it by factors up to 2.4:
+ * a trajectory near a barrier top amplifies ANY fp32 rounding by exp(sqrt(max U'') t)).  Beyond that no
+ * fp32 arithmetic meets 1e-5 after 100 steps: use ABM_FP64 or a smaller dt.  abm_get_accuracy reports
+ * the mode in effect and whether the ensemble is beyond these limits.
  * Ignored in fp64.  Both modes consume the same random stream. */
 enum { ABM_ACCURACY_AUTO = 0, ABM_ACCURACY_FAST = 1, ABM_ACCURACY_PRECISE = 2 };
+/* flag OR-ed into the value abm_get_accuracy returns: some set is stiffer than the mode in effect is
+ * good for (FAST: S > 0.15, PRECISE: S > 0.3), so the fp32 state may deviate from an fp64 integration
+ * by more than 1e-5 after 100 steps */
+#define ABM_ACCURACY_BEYOND_TOLERANCE 0x100u
 
 /* abm_params.rng -- where the uniform words come from.
  *   PHILOX        counter-based Philox4x32-10 keyed by (seed, trajectory, step): BASELINE.json
@@ -94,6 +111,13 @@ enum { ABM_ACCURACY_AUTO = 0, ABM_ACCURACY_FAST = 1, ABM_ACCURACY_PRECISE = 2 };
  *                 A/B of generator cost.  Everything else -- initial state,
  *                 uniform maps, Box-Muller, split-launch bit-identity -- is unchanged. */
 enum { ABM_RNG_PHILOX = 0, ABM_RNG_XORSHIFT128 = 1 };
+
+/* abm_params.step_kernel -- which kernel integrates (results are bit-identical whichever runs).
+ *   AUTO         the library chooses by ensemble size.
+ *   PER_THREAD   always one trajectory per thread (step_kernel).
+ *   SPLIT_WARPS  the warp-specialised kernel (noise warps + integrating warps) wherever it applies
+ *                (fp32, Philox, launches of whole Philox blocks), whatever the ensemble size. */
+enum { ABM_STEP_KERNEL_AUTO = 0, ABM_STEP_KERNEL_PER_THREAD = 1, ABM_STEP_KERNEL_SPLIT_WARPS = 2 };
 
 typedef struct abm_ctx abm_ctx; /* opaque, owned by the library */
 
@@ -108,7 +132,7 @@ typedef struct abm_params {
                                   global step count that is a multiple of K; 0 = never         */
   uint32_t accuracy;       /* RC  fp32 only: ABM_ACCURACY_AUTO | _FAST | _PRECISE (see above)      */
   uint32_t rng;            /* RC  ABM_RNG_PHILOX | ABM_RNG_XORSHIFT128                          */
-  uint32_t reserved;       /*     must be 0                                                    */
+  uint32_t step_kernel;    /* RC  ABM_STEP_KERNEL_AUTO | _PER_THREAD | _SPLIT_WARPS (tuning knob)  */
   double dt;               /* RC  time step                                                    */
   double gamma0, q, c, d, D; /*   Eqs. 1-2                                                     */
   double F0;               /*     constant load force, +F0 as printed in Eq. 2   */
@@ -170,9 +194,14 @@ int abm_moments(abm_ctx* ctx, abm_moment* out);
  * the copy a true asynchronous DMA, pageable memory is staged by the driver. */
 int abm_moments_async(abm_ctx* ctx, abm_moment* out);
 
-/* The raw sums (HOST, out[n_param_sets][ABM_N_SUMS]) and the pure host-side finalisation used
+/* The raw sums (HOST, out[n_param_sets][ABM_N_SUMS]; waits) and the pure host-side finalisation used
  * after summing shards: out_moments[s] from sums[s]. */
 int abm_moment_sums(abm_ctx* ctx, double* out);
+
+/* The same raw sums written to a caller-owned DEVICE buffer dev_out[n_param_sets][ABM_N_SUMS] (8-byte
+ * aligned; e.g. rows of a torch tensor that an NCCL all-reduce then sums across shards):
+ * the reduction and a device-to-device copy are enqueued on the context's stream, nothing waits. */
+int abm_moment_sums_dev(abm_ctx* ctx, double* dev_out);
 int abm_moments_from_sums(const double* sums, uint32_t n_param_sets, uint64_t step,
                           abm_moment* out_moments);
 
@@ -205,18 +234,41 @@ int abm_raster(abm_ctx* ctx, uint32_t* dev_counts, uint32_t width, uint32_t heig
 /* Global step count reached so far. */
 int abm_get_step(const abm_ctx* ctx, uint64_t* out_step);
 
-/* The fp32 accuracy mode in effect (ABM_ACCURACY_FAST or _PRECISE; AUTO is resolved at create). */
+/* The fp32 accuracy mode in effect (ABM_ACCURACY_FAST or _PRECISE; AUTO is resolved at create), OR-ed
+ * with ABM_ACCURACY_BEYOND_TOLERANCE if some set is stiffer than that mode is good for (see above). */
 int abm_get_accuracy(const abm_ctx* ctx, uint32_t* out_mode);
 
-/* Wait for the context's stream and free everything the library owns. */
+/* Wait for the context's stream and free everything the library owns.  ABM_ESTATE for a NULL, never
+ * created or already destroyed handle (nothing is dereferenced). */
 int abm_destroy(abm_ctx* ctx);
 
-/* Diagnostics of the random stream (tests: "bit-exact for the RNG integer stream").
+/* Give the freed device memory the library's pool of the CURRENT device still caches back to the driver
+ * (waits for the device).  Live contexts keep theirs. */
+int abm_trim(void);
+
+/* Diagnostics of the random stream (tests: "bit-exact for the RNG integer stream", BASELINE.json).
  * dev_out[(k * n_blocks + j) * 4 + w] = word w of Philox block block_first + j of trajectory
- * traj_first + k -- produced by the same device function the step kernels call.
- * stream: cudaStream_t or NULL.  Asynchronous. */
+ * traj_first + k.  stream: cudaStream_t or NULL.  Asynchronous.
+ *
+ * abm_philox_blocks computes every block with the plain ten-round function (philox_block), the code the
+ * single-step path, the init / moment kernels and the small-ensemble kernel's noise warps call.
+ *
+ * abm_philox_blocks_loop produces the same words THE WAY THE BLOCK LOOP OF THE STEP KERNELS DOES: it
+ * launches, with abm_step's launch geometry (128 threads, one trajectory per thread), a kernel that
+ * instantiates the very loop function the step kernels run (run_steps) with a body that stores each
+ * block's words instead of integrating with them -- the per-trajectory half of rounds 0-1 done once,
+ * the per-block half fetched from the double-buffered shared-memory table that is refilled every 128
+ * blocks, rounds 2-9 with the round keys the host computes, the look-ahead pipeline, and
+ *   loop_shape 0: two blocks per loop trip (the fp32 kernels), 1: one block per trip (the fp64 kernels);
+ *   frame_every_blocks != 0: the loop is cut into segments of that many blocks as by a frame period of
+ *   4 * frame_every_blocks steps (odd segments exercise the loop's one-block prologue).
+ * A trajectory range that straddles a multiple of 2^32 runs the loop's table-free branch, as in abm_step.
+ * n_blocks <= 2^28; block_first + n_blocks <= 2^62. */
 int abm_philox_blocks(uint64_t seed, uint64_t traj_first, uint64_t n_traj, uint64_t block_first,
                       uint64_t n_blocks, uint32_t* dev_out, void* stream);
+int abm_philox_blocks_loop(uint64_t seed, uint64_t traj_first, uint64_t n_traj, uint64_t block_first,
+                           uint64_t n_blocks, uint32_t loop_shape, uint32_t frame_every_blocks,
+                           uint32_t* dev_out, void* stream);
 
 /* Static, non-owning description of a status code. */
 const char* abm_strerror(int status);

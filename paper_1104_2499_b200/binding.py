@@ -17,8 +17,14 @@ ABM_OK, ABM_EINVAL, ABM_ENOMEM, ABM_ECUDA, ABM_ESTATE = 0, -1, -2, -3, -4
 ABM_FP32, ABM_FP64 = 0, 1
 ABM_EULER_MARUYAMA, ABM_HEUN = 0, 1
 ABM_ACCURACY_AUTO, ABM_ACCURACY_FAST, ABM_ACCURACY_PRECISE = 0, 1, 2
+ABM_ACCURACY_BEYOND_TOLERANCE = 0x100
 ABM_RNG_PHILOX, ABM_RNG_XORSHIFT128 = 0, 1
+ABM_STEP_KERNEL_AUTO, ABM_STEP_KERNEL_PER_THREAD, ABM_STEP_KERNEL_SPLIT_WARPS = 0, 1, 2
 ABM_N_SUMS = 8
+
+# abm_params.step_kernel of records built by make_params when the caller names none.  The GPU tests flip it
+# to run every case through both step kernels (results are bit-identical whichever runs).
+DEFAULT_STEP_KERNEL = ABM_STEP_KERNEL_AUTO
 
 
 class abm_params(C.Structure):
@@ -26,7 +32,7 @@ class abm_params(C.Structure):
     _fields_ = [
         ("struct_size", C.c_uint32), ("precision", C.c_uint32), ("integrator", C.c_uint32),
         ("init_v", C.c_uint32), ("snapshot_every", C.c_uint32), ("accuracy", C.c_uint32),
-        ("rng", C.c_uint32), ("reserved", C.c_uint32),
+        ("rng", C.c_uint32), ("step_kernel", C.c_uint32),
         ("dt", C.c_double), ("gamma0", C.c_double), ("q", C.c_double), ("c", C.c_double),
         ("d", C.c_double), ("D", C.c_double), ("F0", C.c_double), ("A", C.c_double),
         ("omega", C.c_double), ("L", C.c_double), ("A1", C.c_double), ("A2", C.c_double),
@@ -48,8 +54,9 @@ MOMENT_DTYPE = np.dtype([("n", "<u8"), ("step", "<u8"), ("mean_x", "<f8"), ("var
                          ("mean_dx", "<f8"), ("mean_dx2", "<f8"), ("mean_x2", "<f8")])
 
 EXPORTS = ["abm_create", "abm_step", "abm_snapshot", "abm_snapshot_host", "abm_moments", "abm_moments_async",
-           "abm_moment_sums", "abm_moments_from_sums", "abm_time_averaged_velocity", "abm_raster", "abm_get_step", "abm_get_accuracy", "abm_destroy",
-           "abm_philox_blocks", "abm_strerror", "abm_abi_version"]
+           "abm_moment_sums", "abm_moment_sums_dev", "abm_moments_from_sums", "abm_time_averaged_velocity",
+           "abm_raster", "abm_get_step", "abm_get_accuracy", "abm_destroy", "abm_trim", "abm_philox_blocks",
+           "abm_philox_blocks_loop", "abm_strerror", "abm_abi_version"]
 
 _lib = None
 
@@ -77,13 +84,16 @@ def lib():
         L.abm_moments.argtypes = [vp, vp]
         L.abm_moments_async.argtypes = [vp, vp]
         L.abm_moment_sums.argtypes = [vp, vp]
+        L.abm_moment_sums_dev.argtypes = [vp, vp]
         L.abm_moments_from_sums.argtypes = [vp, u32, u64, vp]
         L.abm_time_averaged_velocity.argtypes = [vp, vp]
         L.abm_raster.argtypes = [vp, vp, u32, u32, C.c_double, C.c_double, vp, u32]
         L.abm_get_step.argtypes = [vp, C.POINTER(u64)]
         L.abm_get_accuracy.argtypes = [vp, C.POINTER(u32)]
         L.abm_destroy.argtypes = [vp]
+        L.abm_trim.argtypes = []
         L.abm_philox_blocks.argtypes = [u64, u64, u64, u64, u64, vp, vp]
+        L.abm_philox_blocks_loop.argtypes = [u64, u64, u64, u64, u64, u32, u32, vp, vp]
         for n in EXPORTS[:-2]:
             getattr(L, n).restype = C.c_int
         L.abm_strerror.argtypes = [C.c_int]
@@ -94,7 +104,7 @@ def lib():
     return _lib
 
 
-_PARAM_KEYS = ["precision", "integrator", "init_v", "snapshot_every", "accuracy", "rng", "dt", "gamma0", "q", "c", "d",
+_PARAM_KEYS = ["precision", "integrator", "init_v", "snapshot_every", "accuracy", "rng", "step_kernel", "dt", "gamma0", "q", "c", "d",
                "D", "F0", "A", "omega", "L", "A1", "A2", "phi", "v0", "e0", "traj_base",
                "traj_set_stride"]
 
@@ -105,6 +115,7 @@ def make_params(param_sets, stream=0, **common):
     for s, d in enumerate(param_sets):
         p = arr[s]
         p.struct_size = C.sizeof(abm_params)
+        p.step_kernel = DEFAULT_STEP_KERNEL
         for k in _PARAM_KEYS:
             if k in common:
                 setattr(p, k, common[k])
@@ -165,6 +176,11 @@ def abm_moment_sums(ctx, n_param_sets, out=None):
     return out
 
 
+def abm_moment_sums_dev(ctx, dev_ptr):
+    """Enqueue the reduction and a device-to-device copy of the raw sums [n_param_sets][8] to `dev_ptr`."""
+    _check("abm_moment_sums_dev", lib().abm_moment_sums_dev(ctx, dev_ptr))
+
+
 def abm_moments_from_sums(sums, step):
     sums = np.ascontiguousarray(sums, np.float64)
     out = np.zeros(sums.shape[0], MOMENT_DTYPE)
@@ -199,6 +215,17 @@ def abm_destroy(ctx):
     _check("abm_destroy", lib().abm_destroy(ctx))
 
 
+def abm_trim():
+    _check("abm_trim", lib().abm_trim())
+
+
+def abm_philox_blocks_loop(seed, traj_first, n_traj, block_first, n_blocks, loop_shape, frame_every_blocks,
+                           dev_ptr, stream=0):
+    _check("abm_philox_blocks_loop",
+           lib().abm_philox_blocks_loop(seed, traj_first, n_traj, block_first, n_blocks, loop_shape,
+                                        frame_every_blocks, dev_ptr, stream or None))
+
+
 def abm_philox_blocks(seed, traj_first, n_traj, block_first, n_blocks, dev_ptr, stream=0):
     _check("abm_philox_blocks",
            lib().abm_philox_blocks(seed, traj_first, n_traj, block_first & 0xffffffffffffffff,
@@ -227,7 +254,7 @@ class Ensemble:
     """
 
     def __init__(self, param_sets, n_particles, seed, snapshot_every=0, stream=None,
-                 traj_base=0, traj_set_stride=0, accuracy=ABM_ACCURACY_AUTO, rng=None):
+                 traj_base=0, traj_set_stride=0, accuracy=ABM_ACCURACY_AUTO, rng=None, step_kernel=None):
         import torch
         self._torch = torch
         if not torch.cuda.is_available():
@@ -243,6 +270,8 @@ class Ensemble:
                           traj_set_stride=traj_set_stride, accuracy=accuracy)
             if rng is not None:          # else the parameter records decide (default Philox)
                 common["rng"] = rng
+            if step_kernel is not None:  # else the parameter records, else DEFAULT_STEP_KERNEL
+                common["step_kernel"] = step_kernel
             params = make_params(param_sets, stream=self.stream.cuda_stream, **common)
         self.fp64 = int(params[0].precision) == 1
         self.ctx = abm_create(params, n_particles, self.n_sets, seed)
@@ -274,6 +303,13 @@ class Ensemble:
     def moment_sums(self, out=None):
         return abm_moment_sums(self.ctx, self.n_sets, out)
 
+    def moment_sums_dev(self, out):
+        """Raw sums into rows of a caller-owned float64 CUDA tensor [n_sets, 8] (no host round trip)."""
+        assert out.is_cuda and out.dtype == self._torch.float64 and out.is_contiguous() \
+            and tuple(out.shape) == (self.n_sets, ABM_N_SUMS)
+        abm_moment_sums_dev(self.ctx, out.data_ptr())
+        return out
+
     def raster(self, width, height, v_min, v_max, saturation=0):
         """-> (counts int32-viewed uint32 tensor [height, width], rgba uint8 tensor [height, width, 4] or None);
         device tensors owned by the caller, written on this ensemble's stream."""
@@ -297,7 +333,11 @@ class Ensemble:
 
     @property
     def accuracy(self):
-        return abm_get_accuracy(self.ctx)
+        return abm_get_accuracy(self.ctx) & 0xff
+
+    @property
+    def beyond_tolerance(self):
+        return bool(abm_get_accuracy(self.ctx) & ABM_ACCURACY_BEYOND_TOLERANCE)
 
     @property
     def step_count(self):

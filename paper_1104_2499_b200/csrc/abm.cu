@@ -13,6 +13,7 @@
 #include <mutex>
 #include <new>
 #include <thread>
+#include <unordered_set>
 #include <vector>
 
 #include "abm_kernels.cuh"
@@ -39,9 +40,10 @@ struct abm_ctx {
   uint32_t n_sets;
   bool tilt;
   bool precise;         // fp32 accuracy mode resolved at create (include/abm.h, abm_params.accuracy)
+  bool beyond_tolerance;  // some set is stiffer than that mode is good for (ABM_ACCURACY_BEYOND_TOLERANCE)
   uint64_t n_particles, n_traj, seed, step, traj_base, set_stride;
   double dt, omega;
-  uint64_t small_max_traj;  // ensembles up to this size run step_kernel_small (ABM_SMALL_MAX_TRAJ)
+  uint64_t small_max_traj;  // ensembles up to this size run step_kernel_small (abm_params.step_kernel)
   double tilt_k0, tilt_A;  // what the tilt table holds: k0 + A cos(omega t) of the one set, or (0, 1)
   size_t real_size;
   void *x, *v, *e;      // state, SoA, Real[n_traj]
@@ -116,6 +118,8 @@ Coef<Real> make_coef(const abm_params& p) {
 // config[3], against the 1e-5 of BASELINE.json), so ABM_ACCURACY_AUTO switches to the precise
 // kernels above PRECISE_ABOVE.
 constexpr double PRECISE_ABOVE = 0.15;
+// ... and beyond PRECISE_GOOD_TO even the precise kernels may miss 1e-5 (include/abm.h, "What the modes promise")
+constexpr double PRECISE_GOOD_TO = 0.3;
 double stiffness(const abm_params& p) {
   const double g = 6.283185307179586476925286766559 / p.L;
   return p.dt * g * g * (std::fabs(p.A1) + 4.0 * std::fabs(p.A2));
@@ -159,6 +163,7 @@ bool finite_all(const abm_params& p) {
 struct SetFlags {
   std::atomic<int> tilt{0};   // some set has A != 0
   std::atomic<int> stiff{0};  // some set's stiffness() exceeds PRECISE_ABOVE
+  std::atomic<int> very_stiff{0};  // ... exceeds PRECISE_GOOD_TO
 };
 
 int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets, SetFlags* flags) {
@@ -166,14 +171,15 @@ int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets, Se
   const abm_params& p0 = params[0];
   if (p0.struct_size != sizeof(abm_params)) return ABM_EINVAL;
   if (p0.precision > ABM_FP64 || p0.integrator > ABM_HEUN || p0.init_v > ABM_INIT_V_THERMAL ||
-      p0.accuracy > ABM_ACCURACY_PRECISE || p0.rng > ABM_RNG_XORSHIFT128)
+      p0.accuracy > ABM_ACCURACY_PRECISE || p0.rng > ABM_RNG_XORSHIFT128 ||
+      p0.step_kernel > ABM_STEP_KERNEL_SPLIT_WARPS)
     return ABM_EINVAL;
   std::atomic<int> bad{0};
   parallel_sets(n_sets, [&](uint32_t s0, uint32_t s1) {
-    bool tilt = false, stiff = false;
+    bool tilt = false, stiff = false, very_stiff = false;
     for (uint32_t s = s0; s < s1; ++s) {
       const abm_params& p = params[s];
-      bool ok = p.struct_size == sizeof(abm_params) && p.reserved == 0;
+      bool ok = p.struct_size == sizeof(abm_params) && p.step_kernel == p0.step_kernel;
       ok = ok && p.precision == p0.precision && p.integrator == p0.integrator && p.init_v == p0.init_v &&
            p.accuracy == p0.accuracy && p.rng == p0.rng && p.snapshot_every == p0.snapshot_every &&
            p.dt == p0.dt && p.omega == p0.omega && p.traj_base == p0.traj_base &&
@@ -185,23 +191,37 @@ int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets, Se
         return;
       }
       tilt = tilt || p.A != 0.0;
-      stiff = stiff || stiffness(p) > PRECISE_ABOVE;
+      const double S = stiffness(p);
+      stiff = stiff || S > PRECISE_ABOVE;
+      very_stiff = very_stiff || S > PRECISE_GOOD_TO;
     }
     if (tilt) flags->tilt.store(1, std::memory_order_relaxed);
     if (stiff) flags->stiff.store(1, std::memory_order_relaxed);
+    if (very_stiff) flags->very_stiff.store(1, std::memory_order_relaxed);
   });
   if (bad.load()) return ABM_EINVAL;
   // total trajectory count must fit the kernels' 64-bit indexing and 31-bit grids
   const uint64_t max_traj = static_cast<uint64_t>(0x7fffffffu) * STEP_BLOCK;
   if (n_particles > max_traj / n_sets) return ABM_EINVAL;
   if (p0.traj_set_stride != 0 && p0.traj_set_stride < n_particles) return ABM_EINVAL;
+  // the global index range traj_base + (n_sets - 1) stride + n_particles - 1 must not wrap 2^64 (the
+  // kernels derive the shared high word of the Philox counter from its two ends)
+  const uint64_t stride = p0.traj_set_stride ? p0.traj_set_stride : n_particles;
+  const uint64_t span_sets = static_cast<uint64_t>(n_sets - 1);
+  if (span_sets != 0 && stride > (~0ull - (n_particles - 1)) / span_sets) return ABM_EINVAL;
+  const uint64_t span = span_sets * stride + (n_particles - 1);
+  if (p0.traj_base > ~0ull - span) return ABM_EINVAL;
   return ABM_OK;
 }
 
 // Device memory comes from a stream-ordered pool owned by the library (one per device, kept for
-// the life of the process, never trimmed): after the first context of a given size, abm_create /
-// abm_destroy cost microseconds and do not serialise against other users of the driver.
+// the life of the process): after the first context of a given size, abm_create / abm_destroy cost
+// microseconds and do not serialise against other users of the driver.  The pool keeps at most
+// POOL_KEEP_BYTES of freed memory across synchronisation points (every BASELINE.json config fits);
+// what a larger context leaves behind goes back to the driver -- and so to PyTorch's allocator, which
+// cannot see into this pool -- at the next synchronisation, and abm_trim() releases the rest.
 constexpr int MAX_DEVICES = 64;
+constexpr uint64_t POOL_KEEP_BYTES = 1ull << 30;
 std::mutex g_pool_mutex;
 cudaMemPool_t g_pools[MAX_DEVICES] = {};
 
@@ -218,7 +238,7 @@ cudaError_t pool_for(int device, cudaMemPool_t* out) {
     cudaMemPool_t pool = nullptr;
     cudaError_t e = cudaMemPoolCreate(&pool, &props);
     if (e != cudaSuccess) return e;
-    uint64_t keep = ~0ull;
+    uint64_t keep = POOL_KEEP_BYTES;
     e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
     if (e != cudaSuccess) {
       cudaMemPoolDestroy(pool);
@@ -354,9 +374,11 @@ cudaError_t launch_step_p(const abm_ctx* c, const StepArgs<Real>& a) {
   }
   const uint32_t grid = static_cast<uint32_t>((c->n_traj + STEP_BLOCK - 1) / STEP_BLOCK);
   if (c->n_sets == 1)
-    step_kernel<Real, INTEG, TILT, true, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+    step_kernel<Real, INTEG, TILT, COEF_PARAM, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+  else if (c->n_particles % 32 == 0)  // every warp inside one set (config[2]: 64 realisations = two warps)
+    step_kernel<Real, INTEG, TILT, COEF_WARP, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
   else
-    step_kernel<Real, INTEG, TILT, false, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+    step_kernel<Real, INTEG, TILT, COEF_PER_THREAD, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
   return cudaGetLastError();
 }
 
@@ -388,6 +410,15 @@ const Coef<float>& coef0<float>(const abm_ctx* c) { return c->coef0_f; }
 template <>
 const Coef<double>& coef0<double>(const abm_ctx* c) { return c->coef0_d; }
 
+// Philox round keys k0 + r W0, k1 + r W1 of the launch record (constant-bank operands of the LOP3s)
+template <typename Real>
+void fill_round_keys(StepArgs<Real>& a, uint64_t seed) {
+  for (uint32_t r = 0; r < 10; ++r) {
+    a.rk0[r] = static_cast<uint32_t>(seed) + PHILOX_W0 * r;
+    a.rk1[r] = static_cast<uint32_t>(seed >> 32) + PHILOX_W1 * r;
+  }
+}
+
 template <typename Real>
 int step_impl(abm_ctx* c, uint64_t n_steps) {
   StepArgs<Real> a;
@@ -405,10 +436,7 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
   a.traj_base = c->traj_base;
   a.set_stride = c->set_stride;
   a.seed = c->seed;
-  for (uint32_t r = 0; r < 10; ++r) {
-    a.rk0[r] = static_cast<uint32_t>(c->seed) + PHILOX_W0 * r;
-    a.rk1[r] = static_cast<uint32_t>(c->seed >> 32) + PHILOX_W1 * r;
-  }
+  fill_round_keys(a, c->seed);
   a.snap_every = c->snap_every;
   a.snap_stride = c->snap_stride;
   a.coef0 = coef0<Real>(c);
@@ -461,8 +489,34 @@ int reduce_moments(abm_ctx* c) {
   return ABM_OK;
 }
 
+// Live contexts.  A handle is looked up here before it is dereferenced, so a call on a destroyed (or
+// never created) handle answers ABM_ESTATE instead of reading freed memory.
+std::mutex g_live_mutex;
+std::unordered_set<const abm_ctx*>& live_set() {
+  static std::unordered_set<const abm_ctx*>* s = new std::unordered_set<const abm_ctx*>;  // never destroyed
+  return *s;
+}
+bool is_live(const abm_ctx* c) {
+  if (!c) return false;
+  std::lock_guard<std::mutex> lock(g_live_mutex);
+  return live_set().count(c) != 0;
+}
+bool register_ctx(const abm_ctx* c) {
+  std::lock_guard<std::mutex> lock(g_live_mutex);
+  try {
+    live_set().insert(c);
+  } catch (...) {
+    return false;
+  }
+  return true;
+}
+bool unregister_ctx(const abm_ctx* c) {  // true: it was live (the caller now owns its destruction)
+  std::lock_guard<std::mutex> lock(g_live_mutex);
+  return live_set().erase(c) != 0;
+}
+
 int check_ctx(const abm_ctx* c) {
-  if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
+  if (!is_live(c) || c->magic != CTX_MAGIC) return ABM_ESTATE;
   if (c->sticky) return ABM_ECUDA;
   return ABM_OK;
 }
@@ -543,16 +597,15 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   c->tilt_k0 = n_param_sets == 1 ? (6.283185307179586476925286766559 / p0.L) * 2.0 * p0.A2 + p0.F0 : 0.0;
   c->tilt_A = n_param_sets == 1 ? p0.A : 1.0;
   c->real_size = c->precision == ABM_FP32 ? 4 : 8;
-  c->small_max_traj = ABM_SMALL_MAX_TRAJ;
-  if (const char* env = std::getenv("ABM_SMALL_MAX_TRAJ")) {  // tuning / test knob: results do not depend on it
-    char* end = nullptr;
-    const unsigned long long v = std::strtoull(env, &end, 10);
-    if (end != env) c->small_max_traj = v;
-  }
+  // which step kernel (abm_params.step_kernel; results do not depend on it)
+  c->small_max_traj = p0.step_kernel == ABM_STEP_KERNEL_PER_THREAD    ? 0
+                      : p0.step_kernel == ABM_STEP_KERNEL_SPLIT_WARPS ? ~0ull
+                                                                      : ABM_SMALL_MAX_TRAJ;
   c->precise = false;
   if (c->precision == ABM_FP32) {
     if (p0.accuracy == ABM_ACCURACY_PRECISE) c->precise = true;
     if (p0.accuracy == ABM_ACCURACY_AUTO && flags.stiff.load() != 0) c->precise = true;
+    c->beyond_tolerance = c->precise ? flags.very_stiff.load() != 0 : flags.stiff.load() != 0;
   }
   c->coef0_f = make_coef<float>(p0);
   c->coef0_d = make_coef<double>(p0);
@@ -599,6 +652,10 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   rc = c->precision == ABM_FP32 ? upload_coefs_and_init<float>(c, params)
                                 : upload_coefs_and_init<double>(c, params);
   if (rc != ABM_OK) return fail(rc);
+  if (!register_ctx(c)) {
+    cudaStreamSynchronize(c->stream);
+    return fail(ABM_ENOMEM);
+  }
   *out = c;
   return ABM_OK;
 }
@@ -687,6 +744,18 @@ int abm_moment_sums(abm_ctx* c, double* out) {
   return ABM_OK;
 }
 
+int abm_moment_sums_dev(abm_ctx* c, double* dev_out) {
+  const int st = check_ctx(c);
+  if (st != ABM_OK) return st;
+  const DeviceGuard on_device(c);
+  if (!dev_out || reinterpret_cast<uintptr_t>(dev_out) % 8 != 0) return ABM_EINVAL;
+  const int rc = c->precision == ABM_FP32 ? reduce_moments<float>(c) : reduce_moments<double>(c);
+  if (rc != ABM_OK) return rc;
+  ABM_CK(c, cudaMemcpyAsync(dev_out, c->sums, sizeof(double) * N_SUMS * c->n_sets,
+                            cudaMemcpyDeviceToDevice, c->stream));
+  return ABM_OK;
+}
+
 int abm_raster(abm_ctx* c, uint32_t* dev_counts, uint32_t width, uint32_t height, double v_min,
                double v_max, uint8_t* dev_rgba, uint32_t saturation) {
   const int st = check_ctx(c);
@@ -766,21 +835,22 @@ int abm_moments_from_sums(const double* sums, uint32_t n_param_sets, uint64_t st
 }
 
 int abm_get_step(const abm_ctx* c, uint64_t* out_step) {
-  if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
+  if (!is_live(c)) return ABM_ESTATE;
   if (!out_step) return ABM_EINVAL;
   *out_step = c->step;
   return ABM_OK;
 }
 
 int abm_get_accuracy(const abm_ctx* c, uint32_t* out_mode) {
-  if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
+  if (!is_live(c)) return ABM_ESTATE;
   if (!out_mode) return ABM_EINVAL;
-  *out_mode = c->precise ? ABM_ACCURACY_PRECISE : ABM_ACCURACY_FAST;
+  *out_mode = (c->precise ? ABM_ACCURACY_PRECISE : ABM_ACCURACY_FAST) |
+              (c->beyond_tolerance ? ABM_ACCURACY_BEYOND_TOLERANCE : 0u);
   return ABM_OK;
 }
 
 int abm_destroy(abm_ctx* c) {
-  if (!c || c->magic != CTX_MAGIC) return ABM_ESTATE;
+  if (!unregister_ctx(c)) return ABM_ESTATE;  // null, never created, or destroyed before
   {
     const DeviceGuard on_device(c);
     cudaStreamSynchronize(c->stream);
@@ -803,6 +873,56 @@ int abm_philox_blocks(uint64_t seed, uint64_t traj_first, uint64_t n_traj, uint6
   return cudaGetLastError() == cudaSuccess ? ABM_OK : ABM_ECUDA;
 }
 
+int abm_philox_blocks_loop(uint64_t seed, uint64_t traj_first, uint64_t n_traj, uint64_t block_first,
+                           uint64_t n_blocks, uint32_t loop_shape, uint32_t frame_every_blocks,
+                           uint32_t* dev_out, void* stream) {
+  if (!dev_out || n_traj == 0 || n_blocks == 0 || loop_shape > 1) return ABM_EINVAL;
+  if (reinterpret_cast<uintptr_t>(dev_out) % 16 != 0) return ABM_EINVAL;
+  if (n_blocks > (MAX_LAUNCH_STEPS >> 2) || block_first > (~0ull >> 2) - n_blocks) return ABM_EINVAL;
+  if (frame_every_blocks > (1u << 28)) return ABM_EINVAL;
+  if (n_traj > static_cast<uint64_t>(0x7fffffffu) * STEP_BLOCK || traj_first > ~0ull - (n_traj - 1))
+    return ABM_EINVAL;
+  // the same launch record abm_step builds (step_impl): round keys on the host, shared high word of the
+  // trajectory index when the range does not straddle a multiple of 2^32
+  auto launch = [&](auto real_tag) {
+    using Real = decltype(real_tag);
+    StepArgs<Real> a;
+    std::memset(static_cast<void*>(&a), 0, sizeof(a));
+    a.n_traj = n_traj;
+    a.n_particles = n_traj;
+    a.traj_base = traj_first;
+    a.set_stride = n_traj;
+    a.seed = seed;
+    fill_round_keys(a, seed);
+    a.step0 = block_first << 2;
+    a.tilt_base = a.step0;
+    a.n_steps = static_cast<uint32_t>(n_blocks << 2);
+    a.snap_every = frame_every_blocks << 2;
+    a.snap = frame_every_blocks ? static_cast<void*>(dev_out) : nullptr;  // only compared with null
+    const uint64_t g_last = traj_first + (n_traj - 1);
+    a.traj_hi = static_cast<uint32_t>(traj_first >> 32);
+    a.traj_hi_shared = (traj_first >> 32) == (g_last >> 32) ? 1u : 0u;
+    const uint32_t grid = static_cast<uint32_t>((n_traj + STEP_BLOCK - 1) / STEP_BLOCK);
+    philox_loop_kernel<Real><<<grid, STEP_BLOCK, 0, static_cast<cudaStream_t>(stream)>>>(
+        a, reinterpret_cast<uint4*>(dev_out));
+  };
+  if (loop_shape == 0) launch(float{}); else launch(double{});
+  return cudaGetLastError() == cudaSuccess ? ABM_OK : ABM_ECUDA;
+}
+
+int abm_trim(void) {
+  int device = -1;
+  if (cudaGetDevice(&device) != cudaSuccess || device < 0 || device >= MAX_DEVICES) return ABM_ECUDA;
+  cudaMemPool_t pool = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    pool = g_pools[device];
+  }
+  if (!pool) return ABM_OK;  // nothing was ever allocated on this device
+  if (cudaDeviceSynchronize() != cudaSuccess) return ABM_ECUDA;
+  return cudaMemPoolTrimTo(pool, 0) == cudaSuccess ? ABM_OK : ABM_ECUDA;
+}
+
 const char* abm_strerror(int status) {
   switch (status) {
     case ABM_OK: return "ok";
@@ -814,6 +934,6 @@ const char* abm_strerror(int status) {
   }
 }
 
-uint32_t abm_abi_version(void) { return 5; }
+uint32_t abm_abi_version(void) { return 6; }
 
 }  // extern "C"

@@ -418,14 +418,16 @@ __device__ __forceinline__ double add_(double a, double b) { return __dadd_rn(a,
 // then cos(thb + (2 pi / L) x): the same FFMA as in fast mode with thb in place of the phase.
 // Cost over fast mode: 2 FP32 + 1 F2I + 1 I2F + 2 integer adds per FOUR steps, two more words of
 // state.  (A float -> integer conversion per step would be cheaper on the FMA port but runs at MUFU
-// rate on the pipe the cosines already keep 60 % busy.)  Valid while 4 |v dt| < L / 2.
+// rate on the pipe the cosines already keep 60 % busy.)  The conversion is 64 bits wide, so the offset of
+// four steps may be any number of periods.
 __device__ __forceinline__ float fixed_angle(uint32_t xf, float th_o) {
   // 2 pi 2^-32 * (signed fraction) + phase
   return __fmaf_rn(static_cast<float>(static_cast<int32_t>(xf)), 1.4629180792671596e-09f, th_o);
 }
 __device__ __forceinline__ void fold(State<float>& s, const Coef<float>& k) {
-  const int32_t d = __float2int_rn(__fmul_rn(s.x, k.fxS));
-  const int64_t X = ((static_cast<int64_t>(s.xc) << 32) | s.xf) + static_cast<int64_t>(d);
+  // 64-bit conversion: any offset is legal (a 32-bit one would saturate silently at |offset| >= L / 2)
+  const int64_t d = __float2ll_rn(__fmul_rn(s.x, k.fxS));
+  const int64_t X = ((static_cast<int64_t>(s.xc) << 32) | s.xf) + d;
   s.xf = static_cast<uint32_t>(X);
   s.xc = static_cast<int32_t>(X >> 32);
   s.x = 0.0f;

@@ -31,10 +31,17 @@ namespace abm {
 #define ABM_MINB_F64 5    // fp64: <= 96 regs (ptxas takes 86: no stack traffic in the loop)
 #endif
 constexpr int STEP_BLOCK = ABM_STEP_BLOCK;   // threads per CTA of the step kernel
-template <typename Real, int INTEG, bool UNIFORM>
+// Where a thread's coefficient record comes from.
+//   COEF_PER_THREAD   loaded per thread from the table into vector registers (sets of any size)
+//   COEF_PARAM        one parameter set: the record is a kernel parameter (constant-bank operands)
+//   COEF_WARP         several sets whose size is a multiple of 32: every warp lies inside one set, and its
+//                     record is moved to uniform registers (see warp_uniform)
+enum { COEF_PER_THREAD = 0, COEF_PARAM = 1, COEF_WARP = 2 };
+template <typename Real, int INTEG, int COEF>
 constexpr int step_min_blocks() {
   return sizeof(Real) == 8 ? ABM_MINB_F64
-                           : (!UNIFORM ? ABM_MINB_F32N : (INTEG == 1 ? ABM_MINB_F32H : ABM_MINB_F32U));
+                           : (COEF == COEF_PER_THREAD ? ABM_MINB_F32N
+                                                      : (INTEG == 1 ? ABM_MINB_F32H : ABM_MINB_F32U));
 }
 constexpr int MOM_BLOCK = 256;    // threads per CTA of the moment reduction (max)
 constexpr int MOM_PER_THREAD = 16;
@@ -273,10 +280,61 @@ constexpr int PHILOX_CHUNK = STEP_BLOCK;  // table entries per refill = threads 
 // XS (generator variant, NEXT-4): the words come from the trajectory's xorshift state S instead.
 // S always sits at a pair boundary -- before output 2 (n >> 1) -- when a step starts: whole blocks
 // draw four outputs; a single even step draws its pair from a copy, the odd step after it commits.
-template <typename Real, int INTEG, int TILT, bool PRECISE, bool TABLE, bool XS>
-__device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_t k, const bool active,
-                                          const uint32_t traj_lo, const uint32_t traj_hi,
-                                          const Coef<Real>& cf, State<Real>& s, uint4& S) {
+//
+// BODY: what is done with the words.  The step kernels integrate (Integrate: four steps per block, one step
+// on the slow path, a frame where one is due); the stream diagnostic (philox_loop_kernel, abm_philox_blocks_loop)
+// stores them (DumpWords) -- it instantiates THIS function, so the words it shows are produced by the
+// instructions the step kernels execute: philox_traj, the double-buffered block-head table, philox_finish_rk
+// with the host-computed round keys, two blocks per trip in fp32.
+template <typename Real, int INTEG, int TILT, bool PRECISE>
+struct Integrate {
+  const StepArgs<Real>& a;
+  const Coef<Real>& cf;
+  State<Real>& s;
+  const uint64_t k;
+  const bool active;
+  const Real* tl;
+  __device__ __forceinline__ Integrate(const StepArgs<Real>& a_, const Coef<Real>& cf_, State<Real>& s_,
+                                       uint64_t k_, bool active_)
+      : a(a_), cf(cf_), s(s_), k(k_), active(active_), tl(nullptr) {}
+  // a run of whole blocks starts at step n
+  __device__ __forceinline__ void start(uint64_t n) { tl = TILT ? a.tilt + (n - a.tilt_base) : nullptr; }
+  __device__ __forceinline__ void block(const uint4& w) { four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl); }
+  // step n alone; w holds the words of its pair where the block layout has them
+  __device__ __forceinline__ void single(const uint4& w, uint64_t n) {
+    const Noise4<Real> z(w, cf);
+    const bool second = (n >> 1) & 1u;
+    const Real rho = Noise4<Real>::SIGN * (second ? z.b.rho : z.a.rho);
+    const Real cs = (n & 1u) ? (second ? z.b.sn : z.a.sn) : (second ? z.b.cs : z.a.cs);
+    Real t0 = 0, t1 = 0;
+    if (TILT) {
+      t0 = a.tilt[n - a.tilt_base];
+      if (INTEG == 1) t1 = a.tilt[n - a.tilt_base + 1];
+    }
+    one_step<Real, INTEG, TILT, PRECISE>(s, cf, rho, cs, t0, t1);
+    if constexpr (PRECISE) {
+      if ((n & 3u) == 3u) fold(s, cf);  // the same rule as four_steps
+    }
+  }
+  __device__ __forceinline__ void frame() {
+    if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
+  }
+};
+struct DumpWords {
+  uint4* out;  // the next block of this thread's trajectory (nullptr: a shadowing thread, stores nothing)
+  __device__ __forceinline__ void start(uint64_t) {}
+  __device__ __forceinline__ void block(const uint4& w) {
+    if (out) *out++ = w;
+  }
+  __device__ __forceinline__ void single(const uint4& w, uint64_t n) {
+    if (out && (n & 3u) == 0) *out++ = w;
+  }
+  __device__ __forceinline__ void frame() {}
+};
+
+template <typename Real, bool TABLE, bool XS, typename Body>
+__device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint32_t traj_lo,
+                                          const uint32_t traj_hi, Body& body, uint4& S) {
   __shared__ uint4 tab[TABLE ? 2 : 1][TABLE ? PHILOX_CHUNK : 1];
   uint32_t par = 0;
   const uint32_t k0 = static_cast<uint32_t>(a.seed), k1 = static_cast<uint32_t>(a.seed >> 32);
@@ -301,7 +359,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
       const uint32_t nb = static_cast<uint32_t>(nb64 > 0x40000000ull ? 0x40000000ull : nb64);
       const uint32_t b_hi = static_cast<uint32_t>(b >> 32);
       uint32_t b_lo = static_cast<uint32_t>(b);
-      const Real* tl = TILT ? a.tilt + (n - a.tilt_base) : nullptr;
+      body.start(n);
       uint64_t to_snap = (K && snap_aligned) ? (next_snap - n) >> 2 : ~0ull;  // blocks to the frame
       uint32_t left = nb;
       if (XS) {
@@ -315,28 +373,28 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
           if constexpr (sizeof(Real) == 4 && ABM_UNROLL2 != 0) {  // two blocks per trip, as for Philox
             if (ahead & 1u) {
               const uint4 w_next = xorshift128_x4(S);
-              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+              body.block(w);
               w = w_next;
             }
 #pragma unroll 1
             for (ahead >>= 1; ahead; --ahead) {
               const uint4 wa = xorshift128_x4(S);
-              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+              body.block(w);
               w = xorshift128_x4(S);
-              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, wa, tl);
+              body.block(wa);
             }
           } else {
 #pragma unroll 1
             for (; ahead; --ahead) {
               const uint4 w_next = xorshift128_x4(S);
-              four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+              body.block(w);
               w = w_next;
             }
           }
-          if (last) four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+          if (last) body.block(w);
           left -= seg;
           if (seg == to_snap) {  // a frame is due after this block
-            if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
+            body.frame();
             to_snap = K >> 2;
           } else {
             to_snap -= seg;
@@ -370,7 +428,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
               if (seg & 1u) {
                 const uint4 u = *tp++;
                 const uint4 w_next = PHILOX_FINISH(pt, u, a, k0, k1);
-                four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+                body.block(w);
                 w = w_next;
               }
               const uint4* const tp_end = tp + (seg & ~1u);
@@ -378,10 +436,10 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
               while (tp != tp_end) {
                 const uint4 ua = tp[0];
                 const uint4 wa = PHILOX_FINISH(pt, ua, a, k0, k1);
-                four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+                body.block(w);
                 const uint4 ub = tp[1];
                 w = PHILOX_FINISH(pt, ub, a, k0, k1);
-                four_steps<Real, INTEG, TILT, PRECISE>(s, cf, wa, tl);
+                body.block(wa);
                 tp += 2;
               }
             } else {
@@ -390,13 +448,13 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
               do {
                 const uint4 u = *tp;
                 const uint4 w_next = PHILOX_FINISH(pt, u, a, k0, k1);
-                four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+                body.block(w);
                 w = w_next;
               } while (++tp != tp_end);
             }
             done += seg;
             if (seg == to_snap) {  // a frame is due after this block
-              if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
+              body.frame();
               to_snap = K >> 2;
             } else {
               to_snap -= seg;
@@ -413,12 +471,12 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
 #pragma unroll 1
           do {
             const uint4 w_next = philox4x32_10(b_lo + 1u, b_hi, traj_lo, traj_hi, k0, k1);
-            four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl);
+            body.block(w);
             w = w_next;
           } while (++b_lo != seg_end);
           left -= seg;
           if (seg == to_snap) {  // a frame is due after this block
-            if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
+            body.frame();
             to_snap = K >> 2;
           } else {
             to_snap -= seg;
@@ -441,23 +499,11 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
       } else {
         w = philox_block(a.seed, (static_cast<uint64_t>(traj_hi) << 32) | traj_lo, n >> 2);
       }
-      const Noise4<Real> z(w, cf);
-      const bool second = (n >> 1) & 1u;
-      const Real rho = Noise4<Real>::SIGN * (second ? z.b.rho : z.a.rho);
-      const Real cs = (n & 1u) ? (second ? z.b.sn : z.a.sn) : (second ? z.b.cs : z.a.cs);
-      Real t0 = 0, t1 = 0;
-      if (TILT) {
-        t0 = a.tilt[n - a.tilt_base];
-        if (INTEG == 1) t1 = a.tilt[n - a.tilt_base + 1];
-      }
-      one_step<Real, INTEG, TILT, PRECISE>(s, cf, rho, cs, t0, t1);
-      if constexpr (PRECISE) {
-        if ((n & 3u) == 3u) fold(s, cf);  // the same rule as four_steps
-      }
+      body.single(w, n);
       ++n;
     }
     if (n == next_snap) {
-      if (active) store_snapshot(a.snap, a.snap_stride, k, frame_state<PRECISE>(s, cf));
+      body.frame();
       next_snap += K;
     }
   }
@@ -467,9 +513,23 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint64_
 #define ABM_PHILOX_TABLE 1
 #endif
 
-template <typename Real, int INTEG, bool TILT, bool UNIFORM, bool PRECISE, bool XS>
-__global__ void __launch_bounds__(STEP_BLOCK, step_min_blocks<Real, INTEG, UNIFORM>())
+// A value every lane of the warp holds alike, moved to a uniform register: REDUX (redux.sync) writes its result
+// to the uniform register file, and the minimum over equal words is the word.  ptxas then uses it as the uniform
+// operand of FFMA / LOP3 exactly as it uses a kernel parameter -- which it cannot prove for a value that was
+// loaded through a thread-dependent address.  All 32 lanes must be converged.
+__device__ __forceinline__ float warp_uniform(float v) {
+  return __uint_as_float(__reduce_min_sync(0xffffffffu, __float_as_uint(v)));
+}
+__device__ __forceinline__ double warp_uniform(double v) {
+  const uint32_t lo = __reduce_min_sync(0xffffffffu, static_cast<uint32_t>(__double2loint(v)));
+  const uint32_t hi = __reduce_min_sync(0xffffffffu, static_cast<uint32_t>(__double2hiint(v)));
+  return __hiloint2double(static_cast<int>(hi), static_cast<int>(lo));
+}
+
+template <typename Real, int INTEG, bool TILT, int COEF, bool PRECISE, bool XS>
+__global__ void __launch_bounds__(STEP_BLOCK, step_min_blocks<Real, INTEG, COEF>())
 step_kernel(const __grid_constant__ StepArgs<Real> a) {
+  constexpr bool UNIFORM = COEF == COEF_PARAM;
   const uint64_t k_raw = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
   const bool active = k_raw < a.n_traj;
   const uint64_t k = active ? k_raw : a.n_traj - 1;  // idle threads shadow the last trajectory
@@ -487,6 +547,23 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
     cf.th_o = g->th_o;
     cf.bm_o = g->bm_o;
   }
+  if constexpr (COEF == COEF_WARP) {
+    // The host sends this kernel only when n_particles is a multiple of 32 (and n_traj with it): the lanes
+    // of a warp -- shadowing lanes included -- share one set, so the record is warp-uniform.  The same
+    // operands as above stay in vector registers; the others go to uniform registers.
+    cf.dt = warp_uniform(cf.dt);
+    cf.hdt = warp_uniform(cf.hdt);
+    cf.gamma0 = warp_uniform(cf.gamma0);
+    cf.q = warp_uniform(cf.q);
+    cf.c = warp_uniform(cf.c);
+    cf.k0 = warp_uniform(cf.k0);
+    cf.k2 = warp_uniform(cf.k2);
+    cf.th_s = warp_uniform(cf.th_s);
+    cf.s2 = warp_uniform(cf.s2);
+    cf.A = warp_uniform(cf.A);
+    cf.L = warp_uniform(cf.L);
+    cf.fxS = warp_uniform(cf.fxS);
+  }
 
   State<Real> s{a.x[k], a.v[k], a.e[k], Real(0), 0u, 0, Real(0)};
   if constexpr (PRECISE) {  // x is the offset; the xl / xh arrays hold the fixed-point words
@@ -500,16 +577,15 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
   // straddles a multiple of 2^32); the block-head table of run_steps needs that.
   uint4 S = make_uint4(0u, 0u, 0u, 0u);
   constexpr int TL = TILT ? (UNIFORM ? 2 : 1) : 0;  // what the tilt table holds (one_step)
+  Integrate<Real, INTEG, TL, PRECISE> body(a, cf, s, k, active);
   if (XS) {
     S = a.rng_state[k];
-    run_steps<Real, INTEG, TL, PRECISE, false, true>(a, k, active, 0u, 0u, cf, s, S);
+    run_steps<Real, false, true>(a, 0u, 0u, body, S);
   } else if (a.traj_hi_shared) {
-    run_steps<Real, INTEG, TL, PRECISE, ABM_PHILOX_TABLE != 0, false>(
-        a, k, active, static_cast<uint32_t>(id.global), a.traj_hi, cf, s, S);
+    run_steps<Real, ABM_PHILOX_TABLE != 0, false>(a, static_cast<uint32_t>(id.global), a.traj_hi, body, S);
   } else {
-    run_steps<Real, INTEG, TL, PRECISE, false, false>(
-        a, k, active, static_cast<uint32_t>(id.global), static_cast<uint32_t>(id.global >> 32), cf,
-        s, S);
+    run_steps<Real, false, false>(a, static_cast<uint32_t>(id.global),
+                                  static_cast<uint32_t>(id.global >> 32), body, S);
   }
 
   if (active) {
@@ -811,6 +887,27 @@ __global__ void philox_blocks_kernel(uint64_t seed, uint64_t traj_first, uint64_
   if (t >= n_traj * n_blocks) return;
   const uint64_t k = t / n_blocks, j = t - k * n_blocks;
   out[t] = philox_block(seed, traj_first + k, block_first + j);
+}
+
+// The same words as the block loop of the step kernels produces them: this kernel has step_kernel's launch
+// geometry and thread <-> trajectory assignment and instantiates the SAME run_steps (above) with a body that
+// stores each block's words instead of integrating with them.  a.step0 = 4 * first block, a.n_steps = 4 *
+// blocks, a.snap_every = frame period in steps (segments the loop as frames do; nothing is stored for them),
+// a.snap any non-null pointer if a.snap_every != 0.  out[k * n_blocks + j] = block step0 / 4 + j of trajectory k.
+// Real only selects the loop shape (float: two blocks per trip; double: one).
+template <typename Real>
+__global__ void __launch_bounds__(STEP_BLOCK)
+philox_loop_kernel(const __grid_constant__ StepArgs<Real> a, uint4* __restrict__ out) {
+  const uint64_t k_raw = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
+  const bool active = k_raw < a.n_traj;
+  const uint64_t k = active ? k_raw : a.n_traj - 1;
+  const uint64_t g = a.traj_base + k;
+  DumpWords body{active ? out + k * (a.n_steps >> 2) : nullptr};
+  uint4 S = make_uint4(0u, 0u, 0u, 0u);
+  if (a.traj_hi_shared)
+    run_steps<Real, ABM_PHILOX_TABLE != 0, false>(a, static_cast<uint32_t>(g), a.traj_hi, body, S);
+  else
+    run_steps<Real, false, false>(a, static_cast<uint32_t>(g), static_cast<uint32_t>(g >> 32), body, S);
 }
 
 }  // namespace abm

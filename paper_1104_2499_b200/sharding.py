@@ -10,6 +10,14 @@ rank finalises the same `abm_moment` records with `abm_moments_from_sums`.
                     traj_base=plan.traj_base, traj_set_stride=plan.traj_set_stride)
     ...
     m = reduce_moments(ens.moment_sums(), ens.step_count, plan)     # identical on every rank
+
+or, without any host round trip between the reduction kernel and the collective (NCCL):
+
+    ex = MomentExchange(plan, n_slots=20)                           # device + pinned host buffers
+    for j in range(20):
+        ens.step(1000); ex.enqueue(ens, j)                          # reduction, all-reduce, async copy: no wait
+    torch.cuda.current_stream().synchronize()
+    m = [ex.result(j) for j in range(20)]
 """
 from dataclasses import dataclass
 
@@ -99,3 +107,47 @@ def reduce_moments(sums: np.ndarray, step: int, plan: ShardPlan, group=None, dev
     """Raw sums of this rank -> finalised moments of the whole job (abm_moment records)."""
     from . import binding
     return binding.abm_moments_from_sums(reduce_moment_sums(sums, plan, group, device), step)
+
+
+class MomentExchange:
+    """The exchange of the sharded path kept on the device: `abm_moment_sums_dev` writes this
+    rank's raw sums into its rows of a [n_sets_total, 8] float64 CUDA tensor, one `all_reduce` (NCCL over
+    NVLink) sums the tensor in place across ranks, and an asynchronous copy brings it to pinned host memory --
+    all enqueued on the current stream, nothing waits, so moments every M steps do not stall the integration.
+    `result(slot)` finalises on the host (`abm_moments_from_sums`) after the caller has synchronised.
+
+    backend gloo (rehearsal with ranks sharing one GPU; gloo reduces host tensors): the sums take a synchronous
+    detour through the host, everything else is the same code.  world == 1 skips the collective.
+    """
+
+    def __init__(self, plan: ShardPlan, n_slots: int = 1, group=None, backend: str = "nccl"):
+        import torch
+        self._torch, self.plan, self.group, self.backend = torch, plan, group, backend
+        shape = (n_slots, plan.n_sets_total, 8)
+        self.dev = torch.zeros(shape, dtype=torch.float64, device="cuda")
+        self.host = torch.zeros(shape, dtype=torch.float64, pin_memory=True)
+        self.steps = [0] * n_slots
+
+    def enqueue(self, ens, slot: int):
+        torch, plan = self._torch, self.plan
+        buf = self.dev[slot]
+        if plan.split == "sets" and plan.world > 1:
+            buf.zero_()                           # rows of the other ranks' sets: filled by the all-reduce
+        rows = buf[plan.set_first:plan.set_first + plan.n_sets]
+        ens.moment_sums_dev(rows)
+        self.steps[slot] = ens.step_count
+        if plan.world > 1:
+            import torch.distributed as dist
+            if self.backend == "nccl":
+                dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=self.group)
+            else:
+                t = buf.cpu()
+                dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
+                buf.copy_(t)
+        self.host[slot].copy_(buf, non_blocking=True)
+
+    def result(self, slot: int):
+        """Finalised moments of the whole job (valid once the stream the calls were enqueued on has been
+        synchronised)."""
+        from . import binding
+        return binding.abm_moments_from_sums(self.host[slot].numpy(), self.steps[slot])

@@ -34,7 +34,7 @@ def test_every_declared_symbol_is_exported(abm):
     L = abm.lib()
     for n in names:
         assert getattr(L, n) is not None
-    assert L.abm_abi_version() == 5
+    assert L.abm_abi_version() == 6
 
 
 def test_header_is_plain_c_and_layout_matches_ctypes(abm, tmp_path):
@@ -75,13 +75,30 @@ def test_error_paths_without_device(abm):
     bad[0].struct_size = 8
     assert L.abm_create(bad, 16, 1, 1, C.byref(h)) == abm.ABM_EINVAL
     for key, val in [("dt", 0.0), ("dt", float("nan")), ("L", -1.0), ("D", -0.1), ("precision", 7),
-                     ("integrator", 2)]:
+                     ("integrator", 2), ("step_kernel", 3), ("rng", 2), ("accuracy", 3)]:
         bad = abm.make_params([dict(W.config0().set_params(0), **{key: val})])
         assert L.abm_create(bad, 16, 1, 1, C.byref(h)) == abm.ABM_EINVAL, key
     # run-control fields must agree between sets
     two = abm.make_params([W.config0().set_params(0), dict(W.config0().set_params(0), dt=2e-3)])
     assert L.abm_create(two, 16, 2, 1, C.byref(h)) == abm.ABM_EINVAL
     assert h.value is None                                  # *out untouched on error
+    # the global trajectory index range must not wrap 2^64 (it keys the Philox counter)
+    one = W.config0().set_params(0)
+    wrap = abm.make_params([one], traj_base=2**64 - 10)
+    assert L.abm_create(wrap, 16, 1, 1, C.byref(h)) == abm.ABM_EINVAL
+    wrap3 = abm.make_params([one] * 3, traj_set_stride=2**63)
+    assert L.abm_create(wrap3, 16, 3, 1, C.byref(h)) == abm.ABM_EINVAL
+    fits = abm.make_params([one], traj_base=2**64 - 16)      # last index = 2^64 - 1: legal
+    rc = L.abm_create(fits, 16, 1, 1, C.byref(h))
+    assert rc in (abm.ABM_OK, abm.ABM_ECUDA)                # ECUDA: no device on this box
+    if rc == abm.ABM_OK:
+        assert L.abm_destroy(h) == abm.ABM_OK
+        h = C.c_void_p()
+    junk = (C.c_char * 4096)()                              # an address that never was a context
+    assert L.abm_destroy(C.addressof(junk)) == abm.ABM_ESTATE
+    assert L.abm_step(C.addressof(junk), 1) == abm.ABM_ESTATE
+    assert L.abm_moment_sums_dev(None, None) == abm.ABM_ESTATE
+    assert L.abm_philox_blocks_loop(1, 0, 1, 0, 1, 2, 0, None, None) == abm.ABM_EINVAL
     # null / never-created contexts
     assert L.abm_step(None, 1) == abm.ABM_ESTATE
     assert L.abm_destroy(None) == abm.ABM_ESTATE
@@ -128,6 +145,12 @@ def test_moments_from_sums_matches_numpy(abm):
     assert m["mean_x2"] == pytest.approx((x * x).mean(), rel=1e-12)
     with pytest.raises(abm.AbmError):
         abm.abm_moments_from_sums(np.zeros((1, 8)), 0)
+
+
+def test_library_reads_no_environment_variable():
+    """The kernel choice is a field of abm_params (step_kernel), not an environment variable."""
+    src = open(os.path.join(ROOT, "paper_1104_2499_b200", "csrc", "abm.cu")).read()
+    assert "getenv" not in src
 
 
 def test_product_never_imports_oracle():

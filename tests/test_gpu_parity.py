@@ -38,12 +38,12 @@ def torch():
 def step_kernel_choice(request, monkeypatch):
     """Every test runs twice: with the library's own choice between step_kernel_small (ensembles up to
     8,192 trajectories, launches of whole Philox blocks) and step_kernel, and with step_kernel forced
-    (ABM_SMALL_MAX_TRAJ=0, read at abm_create) -- the small test ensembles would otherwise never reach
-    the kernel the full-size configs run."""
-    if request.param == "one_per_thread":
-        monkeypatch.setenv("ABM_SMALL_MAX_TRAJ", "0")
-    else:
-        monkeypatch.delenv("ABM_SMALL_MAX_TRAJ", raising=False)
+    (abm_params.step_kernel = ABM_STEP_KERNEL_PER_THREAD in every record the binding builds) -- the small
+    test ensembles would otherwise never reach the kernel the full-size configs run."""
+    from paper_1104_2499_b200 import binding
+    monkeypatch.setattr(binding, "DEFAULT_STEP_KERNEL",
+                        binding.ABM_STEP_KERNEL_PER_THREAD if request.param == "one_per_thread"
+                        else binding.ABM_STEP_KERNEL_AUTO)
     return request.param
 
 
@@ -77,6 +77,132 @@ def test_philox_stream_bit_exact(abm, torch, oracle, seed, traj_first, n_traj, b
             b = (block_first + j) & 0xffffffffffffffff
             want = oracle.block(seed, traj_first + k, b)
             assert [int(v) for v in got[k, j]] == want, (k, j)
+
+
+def _oracle_blocks(oracle, seed, traj, block_first, n_blocks):
+    return np.array([oracle.block(seed, traj, (block_first + j) & 0xffffffffffffffff) for j in range(n_blocks)],
+                    dtype=np.uint32)
+
+
+LOOP_CASES = [
+    # seed, traj_first, n_traj, block_first, n_blocks, frame_every_blocks
+    ("cfg1_whole_run", 7, 0, 256, 0, 25_000, 25),              # config[1]: two CTAs, all 100,000 steps, K = 100
+    ("cfg1_last_cta", 7, 1_048_576 - 200, 200, 0, 700, 0),     # config[1]: the last trajectories, ragged CTA
+    ("cfg0", 42, 0, 130, 0, 2_500, 0),                         # config[0]: 10,000 steps
+    ("odd_segments", 99, 0, 129, 5, 1_031, 3),                 # three-block segments: the one-block prologue
+    ("seed64_trajhi", 2**63 + 99, 5 * 2**32 + 3, 300, 2**35 - 100, 300, 0),   # 64-bit seed, key word 1, ctr words 1, 3
+    ("straddle_2^32", 1234, 2**32 - 100, 300, 1_000, 261, 0),  # counter word 3 differs inside the launch: no table
+    ("block_wrap", 5, 0, 129, 2**32 - 130, 260, 7),            # block counter crosses 2^32: the loop is cut there
+]
+
+
+@pytest.mark.parametrize("loop_shape", [0, 1], ids=["two_blocks_per_trip_f32", "one_block_per_trip_f64"])
+@pytest.mark.parametrize("name,seed,traj_first,n_traj,block_first,n_blocks,feb", LOOP_CASES,
+                         ids=[c[0] for c in LOOP_CASES])
+def test_philox_words_of_the_block_loop_bit_exact(abm, torch, oracle, step_kernel_choice, name, seed, traj_first,
+                                                  n_traj, block_first, n_blocks, feb, loop_shape):
+    """The integer stream AS THE HOT LOOP PRODUCES IT (BASELINE.json north_star: "bit-exactly for the RNG integer
+    stream"; Fig. 1 :79): abm_philox_blocks_loop instantiates the step kernels' own loop function
+    (run_steps: per-trajectory half of rounds 0-1, block-head table in shared memory refilled every 128 blocks,
+    rounds 2-9 with host-computed round keys, look-ahead pipeline, two blocks per trip in fp32) with a body that
+    stores the words.  Compared word for word with the oracle's plain Philox4x32-10 and with the library's own
+    plain function (abm_philox_blocks)."""
+    if step_kernel_choice != "auto":
+        pytest.skip("no context involved")
+    out = torch.zeros((n_traj, n_blocks, 4), dtype=torch.int32, device="cuda")
+    abm.abm_philox_blocks_loop(seed, traj_first, n_traj, block_first, n_blocks, loop_shape, feb, out.data_ptr(),
+                               torch.cuda.current_stream().cuda_stream)
+    plain = torch.zeros_like(out)
+    abm.abm_philox_blocks(seed, traj_first, n_traj, block_first, n_blocks, plain.data_ptr(),
+                          torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert torch.equal(out, plain)                  # every word of every trajectory: loop == plain function
+    got = out.cpu().numpy().view(np.uint32)
+    ks = sorted({0, 1, 31, 32, 127, 128, n_traj - 1} & set(range(n_traj)))
+    if n_blocks > 5000:
+        ks = [0, n_traj - 1]
+    for k in ks:                                    # whole runs of single trajectories against the oracle
+        want = _oracle_blocks(oracle, seed, traj_first + k, block_first, n_blocks)
+        assert np.array_equal(got[k], want), (name, k, np.argwhere(got[k] != want)[:4])
+    rng = np.random.default_rng(1)
+    for k, j in zip(rng.integers(0, n_traj, 300), rng.integers(0, n_blocks, 300)):
+        assert [int(v) for v in got[k, j]] == oracle.block(seed, traj_first + int(k), block_first + int(j)), (k, j)
+
+
+CURAND_SRC = r"""
+// Test helper (pin P2 of SURVEY.md 8(c)): the words cuRAND's device Philox4_32_10 generator returns for
+// curand_init(seed, subsequence = trajectory, offset = 4 * block) followed by curand4().  Test-only: the
+// product neither includes nor links cuRAND.
+#include <cstdio>
+#include <cstdlib>
+#include <curand_kernel.h>
+__global__ void words(unsigned long long seed, unsigned long long traj0, int n_traj, unsigned long long b0,
+                      int n_blocks, uint4* out) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n_traj * n_blocks) return;
+  const int k = t / n_blocks, j = t % n_blocks;
+  curandStatePhilox4_32_10_t st;
+  curand_init(seed, traj0 + k, 4ull * (b0 + j), &st);
+  out[t] = curand4(&st);
+}
+int main(int argc, char** argv) {
+  if (argc != 6) return 2;
+  const unsigned long long seed = strtoull(argv[1], 0, 10), traj0 = strtoull(argv[2], 0, 10),
+                           b0 = strtoull(argv[4], 0, 10);
+  const int n_traj = atoi(argv[3]), n_blocks = atoi(argv[5]), n = n_traj * n_blocks;
+  uint4* d;
+  if (cudaMalloc(&d, sizeof(uint4) * n) != cudaSuccess) return 3;
+  words<<<(n + 127) / 128, 128>>>(seed, traj0, n_traj, b0, n_blocks, d);
+  uint4* h = (uint4*)malloc(sizeof(uint4) * n);
+  if (cudaMemcpy(h, d, sizeof(uint4) * n, cudaMemcpyDeviceToHost) != cudaSuccess) return 4;
+  for (int i = 0; i < n; ++i) printf("%u %u %u %u\n", h[i].x, h[i].y, h[i].z, h[i].w);
+  return 0;
+}
+"""
+
+
+@pytest.fixture(scope="module")
+def curand_words(tmp_path_factory):
+    import os
+    import shutil
+    import subprocess
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc is needed to build the cuRAND helper")
+    d = tmp_path_factory.mktemp("curand")
+    src, exe = d / "curand_words.cu", d / "curand_words"
+    src.write_text(CURAND_SRC)
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O1", "-o", str(exe), str(src)], check=True)
+
+    def run(seed, traj0, n_traj, b0, n_blocks):
+        r = subprocess.run([str(exe)] + [str(v) for v in (seed, traj0, n_traj, b0, n_blocks)], check=True,
+                           capture_output=True, text=True)
+        return np.array(r.stdout.split(), dtype=np.uint64).astype(np.uint32).reshape(n_traj, n_blocks, 4)
+    return run
+
+
+@pytest.mark.parametrize("seed,traj0,n_traj,b0,n_blocks", [
+    (7, 0, 40, 0, 30), (42, 4000, 96, 2490, 10), (2**63 + 99, 2**40 + 3, 7, 2**35 + 1, 5),
+    (1234, 2**32 - 5, 10, 2**32 - 3, 6)])
+def test_stream_layout_matches_curand_philox(abm, torch, oracle, curand_words, step_kernel_choice, seed, traj0, n_traj,
+                                             b0, n_blocks):
+    """Pin P2: the stream layout (seed -> key, trajectory -> counter words 2-3, block -> counter words 0-1) is the
+    one of cuRAND's device Philox4_32_10 state with subsequence = trajectory and offset = 4 * block -- an outside
+    implementation of the same definition.  Oracle, plain device function and hot-loop words all equal it."""
+    if step_kernel_choice != "auto":
+        pytest.skip("no context involved")
+    want = curand_words(seed, traj0, n_traj, b0, n_blocks)
+    for k in range(n_traj):
+        for j in range(n_blocks):
+            assert oracle.block(seed, traj0 + k, b0 + j) == [int(v) for v in want[k, j]], (k, j)
+    a = torch.zeros((n_traj, n_blocks, 4), dtype=torch.int32, device="cuda")
+    b = torch.zeros_like(a)
+    s = torch.cuda.current_stream().cuda_stream
+    abm.abm_philox_blocks(seed, traj0, n_traj, b0, n_blocks, a.data_ptr(), s)
+    abm.abm_philox_blocks_loop(seed, traj0, n_traj, b0, n_blocks, 0, 0, b.data_ptr(), s)
+    torch.cuda.synchronize()
+    assert np.array_equal(a.cpu().numpy().view(np.uint32), want)
+    assert np.array_equal(b.cpu().numpy().view(np.uint32), want)
 
 
 def test_normals_consumed_by_the_step_kernel(abm, oracle):
@@ -882,9 +1008,8 @@ def test_small_ensemble_kernel_is_bit_identical(abm, torch, monkeypatch, step_ke
     wl = mk()
     sets = small(wl, n, n_sets)
     got = {}
-    for limit in ("0", "1000000"):
-        monkeypatch.setenv("ABM_SMALL_MAX_TRAJ", limit)
-        with abm.Ensemble(sets, n, wl.seed, snapshot_every=K) as ens:
+    for limit, choice in (("0", abm.ABM_STEP_KERNEL_PER_THREAD), ("1000000", abm.ABM_STEP_KERNEL_SPLIT_WARPS)):
+        with abm.Ensemble(sets, n, wl.seed, snapshot_every=K, step_kernel=choice) as ens:
             frame = ens.bind_snapshot(with_e=True) if K else None
             if name.endswith("_odd"):
                 ens.step(1)
@@ -925,3 +1050,82 @@ def test_more_than_2_to_31_trajectories(abm, torch, oracle, step_kernel_choice):
     assert np.all(np.abs(got - want) <= 1e-6 * np.maximum(1.0, np.abs(want))), np.abs(got - want).max()
     del frame
     torch.cuda.empty_cache()
+
+
+# ---------------------------------------------------------------------------------------------
+# handle lifetime, memory pool, precise-mode fold at any speed
+# ---------------------------------------------------------------------------------------------
+
+def test_calls_after_destroy_answer_estate(abm, torch):
+    """A destroyed handle is looked up in the table of live contexts, never dereferenced (include/abm.h)."""
+    import ctypes as C
+    wl = W.config0()
+    L = abm.lib()
+    ens = abm.Ensemble([wl.set_params(0)], 64, wl.seed)
+    ens.step(4)
+    h = C.c_void_p(ens.ctx.value)
+    assert L.abm_destroy(h) == abm.ABM_OK
+    ens.ctx = None
+    n, m = C.c_uint64(), C.c_uint32()
+    buf = torch.zeros(64 * 8, dtype=torch.float64, device="cuda")
+    assert L.abm_destroy(h) == abm.ABM_ESTATE                   # a second destroy
+    assert L.abm_step(h, 4) == abm.ABM_ESTATE
+    assert L.abm_snapshot(h, buf.data_ptr(), 8) == abm.ABM_ESTATE
+    assert L.abm_moments(h, buf.data_ptr()) == abm.ABM_ESTATE
+    assert L.abm_moment_sums_dev(h, buf.data_ptr()) == abm.ABM_ESTATE
+    assert L.abm_get_step(h, C.byref(n)) == abm.ABM_ESTATE
+    assert L.abm_get_accuracy(h, C.byref(m)) == abm.ABM_ESTATE
+    junk = (C.c_char * 4096)()                                  # an address that never was a context
+    assert L.abm_destroy(C.addressof(junk)) == abm.ABM_ESTATE
+    assert L.abm_step(C.addressof(junk), 1) == abm.ABM_ESTATE
+
+
+def test_trim_releases_the_pool_and_contexts_survive(abm, torch):
+    wl = W.config0()
+    p = [wl.set_params(0)]
+    with abm.Ensemble(p, 50_000, wl.seed) as keep:
+        keep.step(8)
+        before = keep.state()
+        with abm.Ensemble(p, 3_000_000, wl.seed) as big:
+            big.step(4)
+        abm.abm_trim()
+        assert np.array_equal(before, keep.state())             # a live context keeps its memory
+        keep.step(8)
+    with abm.Ensemble(p, 50_000, wl.seed) as again:             # and the pool serves new contexts after a trim
+        again.step(16)
+        with abm.Ensemble(p, 50_000, wl.seed) as ref:
+            ref.step(16)
+            assert np.array_equal(again.state(), ref.state())
+
+
+@pytest.mark.parametrize("v0", [125.0, 400.0, -3000.0], ids=["L/8_per_step", "beyond_L/2_per_block", "3L_per_step"])
+@pytest.mark.parametrize("integrator", [0, 1], ids=["em", "heun"])
+def test_precise_mode_fold_at_any_speed(abm, oracle, v0, integrator):
+    """PRECISE mode folds the four-step float offset into the fixed-point position with a 64-bit conversion: a
+    fast trajectory (|v| dt of L/8, and far beyond the L/2 per block at which a 32-bit conversion saturates) must
+    still follow the oracle.  Free flight with weak damping keeps the speed for the whole run."""
+    p = dict(W.DEFAULTS, integrator=integrator, gamma0=0.01, d=0.0, q=0.0, c=0.1, D=0.01, A1=0.3, A2=0.05, v0=v0)
+    n, seed, steps = 300, 17, 100
+    with abm.Ensemble([p], n, seed, accuracy=abm.ABM_ACCURACY_PRECISE) as ens:
+        assert ens.accuracy == abm.ABM_ACCURACY_PRECISE and not ens.beyond_tolerance
+        ens.step(37)
+        ens.step(63)
+        got = ens.state()
+    x, v, e = oracle.init_many(p, seed, n)
+    oracle.run(p, seed, x, v, e, 0, steps)
+    want = np.stack([x, v, e], 1)
+    assert abs(want[:, 0]).min() > 0.09 * abs(v0)               # they really moved ~ v0 * 100 dt
+    err = scale_rel_err(got[:, :2], want[:, :2])
+    assert np.all(err <= TOL_F32), err
+
+
+def test_accuracy_report_flags_sets_beyond_the_tolerance(abm):
+    base = W.config0().set_params(0)                            # S = 0.079
+    for over, acc, mode, beyond in [
+            ({}, abm.ABM_ACCURACY_AUTO, abm.ABM_ACCURACY_FAST, False),
+            (dict(dt=5e-3), abm.ABM_ACCURACY_AUTO, abm.ABM_ACCURACY_PRECISE, True),     # config[3]'s 0.39
+            (dict(dt=3e-3), abm.ABM_ACCURACY_AUTO, abm.ABM_ACCURACY_PRECISE, False),    # 0.24
+            (dict(dt=3e-3), abm.ABM_ACCURACY_FAST, abm.ABM_ACCURACY_FAST, True),
+            (dict(precision=1, dt=5e-3), abm.ABM_ACCURACY_AUTO, abm.ABM_ACCURACY_FAST, False)]:   # fp64: no modes
+        with abm.Ensemble([dict(base, **over)], 32, 1, accuracy=acc) as ens:
+            assert (ens.accuracy, ens.beyond_tolerance) == (mode, beyond), over

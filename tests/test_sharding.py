@@ -139,3 +139,64 @@ def test_two_gloo_ranks_reduce_to_the_undivided_ensemble(name, oracle):
         assert int(m[s]["n"]) == n_tot and int(m[s]["step"]) == n_steps
         for k, val in want.items():
             assert abs(m[s][k] - val) <= 1e-12 * max(1.0, abs(val)), (name, s, k, m[s][k], val)
+
+
+# ---- the device-side exchange (MomentExchange) with two ranks on the GPU box -----------------------
+
+def _gpu_rank_main(rank, world, port, case, q):
+    import torch
+    import torch.distributed as dist
+    from paper_1104_2499_b200 import binding as abm
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)      # one GPU on the box: the ranks share it
+    try:
+        torch.cuda.set_device(0)
+        n_particles, sets, seed, chunks, scaling = case
+        plan = sharding.shard_plan(n_particles, len(sets), rank, world, scaling)
+        ex = sharding.MomentExchange(plan, n_slots=len(chunks), backend="gloo")
+        mine = sets[plan.set_first:plan.set_first + plan.n_sets]
+        with abm.Ensemble(mine, plan.n_particles, seed, traj_base=plan.traj_base,
+                          traj_set_stride=plan.traj_set_stride) as ens:
+            for j, n in enumerate(chunks):
+                ens.step(n)
+                ex.enqueue(ens, j)                                     # nothing waits here
+            torch.cuda.current_stream().synchronize()
+        q.put((rank, [ex.result(j).tobytes() for j in range(len(chunks))]))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["strong_particles", "strong_sets", "weak_replicas"])
+def test_two_ranks_device_side_exchange_equals_one_context(name):
+    """The sharded job's moments (two contexts on disjoint index ranges, sums exchanged by MomentExchange) against
+    ONE context holding the whole ensemble: same trajectories bit for bit, so the moments agree to the rounding
+    of the differently ordered fp64 sums."""
+    import torch
+    import torch.multiprocessing as mp
+    from paper_1104_2499_b200 import binding as abm
+    assert torch.cuda.is_available()
+    n_particles, sets, seed, n_steps, scaling = _cases()[name]
+    chunks = [n_steps // 2, n_steps - n_steps // 2]
+    case = (n_particles, sets, seed, chunks, scaling)
+    world = 2
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_gpu_rank_main, args=(r, world, port, case, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    results = dict(q.get(timeout=300) for _ in range(world))
+    for p in procs:
+        p.join(60)
+        assert p.exitcode == 0
+    assert results[0] == results[1]                                    # every rank holds the job's moments
+    n_tot = n_particles * (world if scaling == "weak" else 1)
+    with abm.Ensemble(sets, n_tot, seed) as whole:
+        for j, n in enumerate(chunks):
+            whole.step(n)
+            want = whole.moments()
+            got = np.frombuffer(results[0][j], abm.MOMENT_DTYPE)
+            assert np.array_equal(got["n"], want["n"]) and np.array_equal(got["step"], want["step"])
+            for k in ("mean_x", "var_x", "mean_v", "var_v", "mean_e", "mean_dx", "mean_dx2", "mean_x2"):
+                assert np.allclose(got[k], want[k], rtol=1e-12, atol=1e-13), (name, j, k)
