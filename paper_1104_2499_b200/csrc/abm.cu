@@ -40,6 +40,7 @@ struct abm_ctx {
   uint32_t n_sets;
   bool tilt;
   bool precise;         // fp32 accuracy mode resolved at create (include/abm.h, abm_params.accuracy)
+  bool split_coefs;     // several sets that differ only in D, q, F0, A, v0, e0: COEF_SPLIT step kernel
   bool beyond_tolerance;  // some set is stiffer than that mode is good for (ABM_ACCURACY_BEYOND_TOLERANCE)
   uint64_t n_particles, n_traj, seed, step, traj_base, set_stride;
   double dt, omega;
@@ -164,6 +165,7 @@ struct SetFlags {
   std::atomic<int> tilt{0};   // some set has A != 0
   std::atomic<int> stiff{0};  // some set's stiffness() exceeds PRECISE_ABOVE
   std::atomic<int> very_stiff{0};  // ... exceeds PRECISE_GOOD_TO
+  std::atomic<int> shape_differs{0};  // some set differs from set 0 in more than D, q, F0, A, v0, e0
 };
 
 int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets, SetFlags* flags) {
@@ -176,7 +178,7 @@ int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets, Se
     return ABM_EINVAL;
   std::atomic<int> bad{0};
   parallel_sets(n_sets, [&](uint32_t s0, uint32_t s1) {
-    bool tilt = false, stiff = false, very_stiff = false;
+    bool tilt = false, stiff = false, very_stiff = false, shape_differs = false;
     for (uint32_t s = s0; s < s1; ++s) {
       const abm_params& p = params[s];
       bool ok = p.struct_size == sizeof(abm_params) && p.step_kernel == p0.step_kernel;
@@ -191,6 +193,8 @@ int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets, Se
         return;
       }
       tilt = tilt || p.A != 0.0;
+      shape_differs = shape_differs || p.gamma0 != p0.gamma0 || p.c != p0.c || p.d != p0.d || p.L != p0.L ||
+                      p.A1 != p0.A1 || p.A2 != p0.A2 || p.phi != p0.phi;
       const double S = stiffness(p);
       stiff = stiff || S > PRECISE_ABOVE;
       very_stiff = very_stiff || S > PRECISE_GOOD_TO;
@@ -198,6 +202,7 @@ int validate(const abm_params* params, uint64_t n_particles, uint32_t n_sets, Se
     if (tilt) flags->tilt.store(1, std::memory_order_relaxed);
     if (stiff) flags->stiff.store(1, std::memory_order_relaxed);
     if (very_stiff) flags->very_stiff.store(1, std::memory_order_relaxed);
+    if (shape_differs) flags->shape_differs.store(1, std::memory_order_relaxed);
   });
   if (bad.load()) return ABM_EINVAL;
   // total trajectory count must fit the kernels' 64-bit indexing and 31-bit grids
@@ -375,8 +380,8 @@ cudaError_t launch_step_p(const abm_ctx* c, const StepArgs<Real>& a) {
   const uint32_t grid = static_cast<uint32_t>((c->n_traj + STEP_BLOCK - 1) / STEP_BLOCK);
   if (c->n_sets == 1)
     step_kernel<Real, INTEG, TILT, COEF_PARAM, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
-  else if (c->n_particles % 32 == 0)  // every warp inside one set (config[2]: 64 realisations = two warps)
-    step_kernel<Real, INTEG, TILT, COEF_WARP, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
+  else if (c->split_coefs)  // the sets differ only in D, q, F0, A (config[2])
+    step_kernel<Real, INTEG, TILT, COEF_SPLIT, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
   else
     step_kernel<Real, INTEG, TILT, COEF_PER_THREAD, PRECISE, XS><<<grid, STEP_BLOCK, 0, c->stream>>>(a);
   return cudaGetLastError();
@@ -435,6 +440,7 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
   a.n_particles = c->n_particles;
   a.traj_base = c->traj_base;
   a.set_stride = c->set_stride;
+  a.set_magic = set_magic_of(c->n_particles);
   a.seed = c->seed;
   fill_round_keys(a, c->seed);
   a.snap_every = c->snap_every;
@@ -601,6 +607,7 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   c->small_max_traj = p0.step_kernel == ABM_STEP_KERNEL_PER_THREAD    ? 0
                       : p0.step_kernel == ABM_STEP_KERNEL_SPLIT_WARPS ? ~0ull
                                                                       : ABM_SMALL_MAX_TRAJ;
+  c->split_coefs = n_param_sets > 1 && flags.shape_differs.load() == 0;
   c->precise = false;
   if (c->precision == ABM_FP32) {
     if (p0.accuracy == ABM_ACCURACY_PRECISE) c->precise = true;
@@ -892,6 +899,7 @@ int abm_philox_blocks_loop(uint64_t seed, uint64_t traj_first, uint64_t n_traj, 
     a.n_particles = n_traj;
     a.traj_base = traj_first;
     a.set_stride = n_traj;
+    a.set_magic = set_magic_of(n_traj);
     a.seed = seed;
     fill_round_keys(a, seed);
     a.step0 = block_first << 2;

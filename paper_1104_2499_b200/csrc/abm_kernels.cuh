@@ -27,20 +27,28 @@ namespace abm {
 #ifndef ABM_MINB_F32N
 #define ABM_MINB_F32N 4   // fp32, per-thread coefficient record (config[2]): <= 128 regs
 #endif
+#ifndef ABM_MINB_F32S
+#define ABM_MINB_F32S 5   // fp32, sweep over D, q, F0, A only (config[2]): <= 96 regs
+#endif
 #ifndef ABM_MINB_F64
 #define ABM_MINB_F64 5    // fp64: <= 96 regs (ptxas takes 86: no stack traffic in the loop)
 #endif
 constexpr int STEP_BLOCK = ABM_STEP_BLOCK;   // threads per CTA of the step kernel
 // Where a thread's coefficient record comes from.
-//   COEF_PER_THREAD   loaded per thread from the table into vector registers (sets of any size)
+//   COEF_PER_THREAD   the whole record loaded per thread from the table into vector registers (any sweep)
 //   COEF_PARAM        one parameter set: the record is a kernel parameter (constant-bank operands)
-//   COEF_WARP         several sets whose size is a multiple of 32: every warp lies inside one set, and its
-//                     record is moved to uniform registers (see warp_uniform)
-enum { COEF_PER_THREAD = 0, COEF_PARAM = 1, COEF_WARP = 2 };
+//   COEF_SPLIT        a sweep whose sets differ only in D, q, F0, A (noise level, pumping rate, load force, tilt
+//                     amplitude: what the paper, and BASELINE.json configs[2] sweep): the
+//                     coefficients those decide -- s2, q, k0, A -- are loaded per thread, all others are the
+//                     kernel-parameter record of set 0, as in COEF_PARAM.  The same intrinsics on the same
+//                     values as COEF_PER_THREAD: bit-identical results, fewer registers and no round-key
+//                     reloads in the loop.
+enum { COEF_PER_THREAD = 0, COEF_PARAM = 1, COEF_SPLIT = 2 };
 template <typename Real, int INTEG, int COEF>
 constexpr int step_min_blocks() {
   return sizeof(Real) == 8 ? ABM_MINB_F64
                            : (COEF == COEF_PER_THREAD ? ABM_MINB_F32N
+                              : COEF == COEF_SPLIT    ? ABM_MINB_F32S
                                                       : (INTEG == 1 ? ABM_MINB_F32H : ABM_MINB_F32U));
 }
 constexpr int MOM_BLOCK = 256;    // threads per CTA of the moment reduction (max)
@@ -61,6 +69,7 @@ struct StepArgs {
   uint64_t n_traj;               // local trajectories
   uint64_t n_particles;          // per set
   uint64_t traj_base, set_stride;
+  uint64_t set_magic;            // ceil(2^64 / n_particles) (set_magic_of)
   uint64_t seed;
   uint64_t step0;                // first global step of this launch
   uint64_t tilt_base;            // global step of tilt[0]
@@ -80,14 +89,36 @@ struct TrajId {
   uint64_t global;  // index into the random stream
   uint32_t set;
 };
+// global index and set of local trajectory k, with a plain division (kernels that run once)
+__device__ __forceinline__ TrajId traj_id_div(uint64_t k, uint64_t n_particles, uint64_t traj_base,
+                                              uint64_t set_stride, bool single_set) {
+  TrajId t;
+  const uint64_t s = single_set ? 0 : k / n_particles;
+  t.set = static_cast<uint32_t>(s);
+  t.global = traj_base + s * set_stride + (k - s * n_particles);
+  return t;
+}
+// The step kernels: k / n_particles without the 64-bit division subroutine: set_magic = ceil(2^64 / n_particles) from the host
+// (0 stands for 2^64, i.e. n_particles = 1), one high multiply and a correction (the estimate is never low and
+// at most one too high).  A CALL in the step kernels' prologue makes ptxas reload every uniform register --
+// round keys and coefficients -- inside the hot loop (12 LDCU per trip measured).
+__host__ __device__ inline uint64_t set_magic_of(uint64_t n_particles) {
+  return n_particles > 1 ? ~0ull / n_particles + 1 : 0;
+}
+__device__ __forceinline__ uint64_t set_of(uint64_t k, uint64_t n_particles, uint64_t set_magic) {
+  if (set_magic == 0) return k;
+  uint64_t s = __umul64hi(k, set_magic);
+  if (s * n_particles > k) --s;
+  return s;
+}
 __device__ __forceinline__ TrajId traj_id(uint64_t k, uint64_t n_particles, uint64_t traj_base,
-                                          uint64_t set_stride, bool single_set) {
+                                          uint64_t set_stride, bool single_set, uint64_t set_magic) {
   TrajId t;
   if (single_set) {
     t.set = 0;
     t.global = traj_base + k;
   } else {
-    const uint64_t s = k / n_particles;
+    const uint64_t s = set_of(k, n_particles, set_magic);
     t.set = static_cast<uint32_t>(s);
     t.global = traj_base + s * set_stride + (k - s * n_particles);
   }
@@ -147,7 +178,7 @@ __global__ void init_kernel(Real* __restrict__ x, Real* __restrict__ v, Real* __
                             Real* __restrict__ xh) {
   const uint64_t k = static_cast<uint64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
   if (k >= n_traj) return;
-  const TrajId id = traj_id(k, n_particles, traj_base, set_stride, n_sets == 1);
+  const TrajId id = traj_id_div(k, n_particles, traj_base, set_stride, n_sets == 1);
   if (rng_state) rng_state[k] = xorshift_seed(seed, id.global);
   const Coef<Real> c = coef_table[id.set];
   const uint4 w = philox_block(seed, id.global, INIT_BLOCK);
@@ -513,19 +544,6 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint32_
 #define ABM_PHILOX_TABLE 1
 #endif
 
-// A value every lane of the warp holds alike, moved to a uniform register: REDUX (redux.sync) writes its result
-// to the uniform register file, and the minimum over equal words is the word.  ptxas then uses it as the uniform
-// operand of FFMA / LOP3 exactly as it uses a kernel parameter -- which it cannot prove for a value that was
-// loaded through a thread-dependent address.  All 32 lanes must be converged.
-__device__ __forceinline__ float warp_uniform(float v) {
-  return __uint_as_float(__reduce_min_sync(0xffffffffu, __float_as_uint(v)));
-}
-__device__ __forceinline__ double warp_uniform(double v) {
-  const uint32_t lo = __reduce_min_sync(0xffffffffu, static_cast<uint32_t>(__double2loint(v)));
-  const uint32_t hi = __reduce_min_sync(0xffffffffu, static_cast<uint32_t>(__double2hiint(v)));
-  return __hiloint2double(static_cast<int>(hi), static_cast<int>(lo));
-}
-
 template <typename Real, int INTEG, bool TILT, int COEF, bool PRECISE, bool XS>
 __global__ void __launch_bounds__(STEP_BLOCK, step_min_blocks<Real, INTEG, COEF>())
 step_kernel(const __grid_constant__ StepArgs<Real> a) {
@@ -533,9 +551,9 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
   const uint64_t k_raw = static_cast<uint64_t>(blockIdx.x) * STEP_BLOCK + threadIdx.x;
   const bool active = k_raw < a.n_traj;
   const uint64_t k = active ? k_raw : a.n_traj - 1;  // idle threads shadow the last trajectory
-  const TrajId id = traj_id(k, a.n_particles, a.traj_base, a.set_stride, UNIFORM);
-  Coef<Real> cf = UNIFORM ? a.coef0 : a.coef_table[id.set];
-  if (UNIFORM) {
+  const TrajId id = traj_id(k, a.n_particles, a.traj_base, a.set_stride, UNIFORM, a.set_magic);
+  Coef<Real> cf = COEF == COEF_PER_THREAD ? a.coef_table[id.set] : a.coef0;
+  if (COEF != COEF_PER_THREAD) {
     // Kernel-parameter coefficients are uniform operands and an FMA takes at most one of those.
     // One operand of each uniform pair -- (d, c), (d, gamma0), (k2, k1), (th_s, th_o) -- and the
     // Box-Muller angle offset are therefore read from the table in global memory instead: a
@@ -547,22 +565,12 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
     cf.th_o = g->th_o;
     cf.bm_o = g->bm_o;
   }
-  if constexpr (COEF == COEF_WARP) {
-    // The host sends this kernel only when n_particles is a multiple of 32 (and n_traj with it): the lanes
-    // of a warp -- shadowing lanes included -- share one set, so the record is warp-uniform.  The same
-    // operands as above stay in vector registers; the others go to uniform registers.
-    cf.dt = warp_uniform(cf.dt);
-    cf.hdt = warp_uniform(cf.hdt);
-    cf.gamma0 = warp_uniform(cf.gamma0);
-    cf.q = warp_uniform(cf.q);
-    cf.c = warp_uniform(cf.c);
-    cf.k0 = warp_uniform(cf.k0);
-    cf.k2 = warp_uniform(cf.k2);
-    cf.th_s = warp_uniform(cf.th_s);
-    cf.s2 = warp_uniform(cf.s2);
-    cf.A = warp_uniform(cf.A);
-    cf.L = warp_uniform(cf.L);
-    cf.fxS = warp_uniform(cf.fxS);
+  if (COEF == COEF_SPLIT) {  // what differs between the sets of this sweep
+    const Coef<Real>* g = a.coef_table + id.set;
+    cf.s2 = g->s2;
+    cf.q = g->q;
+    cf.k0 = g->k0;
+    cf.A = g->A;
   }
 
   State<Real> s{a.x[k], a.v[k], a.e[k], Real(0), 0u, 0, Real(0)};
@@ -626,7 +634,7 @@ step_kernel_small(const __grid_constant__ StepArgs<float> a) {
   const uint64_t k_raw = static_cast<uint64_t>(blockIdx.x) * SMALL_TRAJ + lane;
   const bool active = k_raw < a.n_traj;
   const uint64_t k = active ? k_raw : a.n_traj - 1;  // idle lanes shadow the last trajectory
-  const TrajId id = traj_id(k, a.n_particles, a.traj_base, a.set_stride, UNIFORM);
+  const TrajId id = traj_id(k, a.n_particles, a.traj_base, a.set_stride, UNIFORM, a.set_magic);
   const Coef<float> cf = UNIFORM ? a.coef0 : a.coef_table[id.set];
   constexpr int TL = TILT ? (UNIFORM ? 2 : 1) : 0;
 

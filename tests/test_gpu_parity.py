@@ -1129,3 +1129,37 @@ def test_accuracy_report_flags_sets_beyond_the_tolerance(abm):
             (dict(precision=1, dt=5e-3), abm.ABM_ACCURACY_AUTO, abm.ABM_ACCURACY_FAST, False)]:   # fp64: no modes
         with abm.Ensemble([dict(base, **over)], 32, 1, accuracy=acc) as ens:
             assert (ens.accuracy, ens.beyond_tolerance) == (mode, beyond), over
+
+
+# ---------------------------------------------------------------------------------------------
+# COEF_SPLIT (sweeps over D, q, F0, A only: s2, q, k0, A per thread, the rest kernel parameters) against
+# COEF_PER_THREAD (any sweep: the whole record per thread): the same intrinsics on the same values
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("integrator,acc,rng,tilt", [(0, 1, 0, 0.0), (0, 2, 0, 0.3), (1, 1, 0, 0.3), (1, 2, 0, 0.0),
+                                                     (0, 1, 1, 0.0), (1, 2, 1, 0.3)],
+                         ids=["em_fast", "em_precise_tilt", "heun_fast_tilt", "heun_precise", "em_xorshift",
+                              "heun_precise_tilt_xorshift"])
+@pytest.mark.parametrize("n_particles", [64, 37], ids=["64", "ragged37"])
+def test_split_coefficient_kernel_is_bit_identical(abm, torch, integrator, acc, rng, tilt, n_particles):
+    """A sweep whose sets differ only in D, q, F0, A runs the COEF_SPLIT kernel; appending one set with another
+    gamma0 sends the SAME sets through COEF_PER_THREAD (the global indices of the first sets do not move).
+    State, frames and moments of the common sets must agree bit for bit."""
+    wl = W.config2(n_D=4, n_q=5, realisations=n_particles)
+    sets = [dict(wl.set_params(s), integrator=integrator, rng=rng, F0=0.02 * s - 0.1, A=tilt * (1 + s % 3),
+                 omega=1.7, dt=2e-3) for s in range(wl.n_param_sets)]
+    odd = dict(sets[3], gamma0=1.25)
+    n_common = len(sets) * n_particles
+    with abm.Ensemble(sets, n_particles, wl.seed, snapshot_every=8, accuracy=acc) as a, \
+            abm.Ensemble(sets + [odd], n_particles, wl.seed, snapshot_every=8, accuracy=acc) as b:
+        fa, fb = a.bind_snapshot(with_e=True), b.bind_snapshot(with_e=True)
+        for n in (1, 120, 83):
+            a.step(n)
+            b.step(n)
+        sa, sb = a.state(), b.state()
+        ma, mb = a.moments(), b.moments()
+        torch.cuda.synchronize()
+        assert np.array_equal(sa, sb[:n_common])
+        assert torch.equal(fa, fb[:n_common])
+        assert np.array_equal(ma.view(np.uint8), mb[:len(sets)].view(np.uint8))
+        assert not np.array_equal(sb[3 * n_particles:4 * n_particles, 1], sb[n_common:, 1])   # gamma0 matters
