@@ -53,6 +53,7 @@ struct abm_ctx {
   uint4* rng_state;     // xorshift state per trajectory (ABM_RNG_XORSHIFT128 only)
   void* coef_table;     // Coef<Real>[n_sets]
   void* tilt_table;     // Real[TILT_CHUNK + 1]
+  double2* noise_tables;  // fp64 only: Box-Muller circle and log tables (NoiseTables), [NOISE_TABLE_N]
   double* partial;      // [n_sets * blocks_per_set][7]
   double* sums;         // [n_sets][8]
   MomentRec* moments;   // [n_sets]
@@ -267,8 +268,8 @@ void dev_free(abm_ctx* c, void* p) {
 }
 
 void free_all(abm_ctx* c) {
-  void* all[] = {c->x, c->v, c->e, c->xl, c->xh, c->rng_state, c->coef_table, c->tilt_table, c->partial, c->sums,
-                 c->moments, c->frame};
+  void* all[] = {c->x, c->v, c->e, c->xl, c->xh, c->rng_state, c->coef_table, c->tilt_table, c->noise_tables,
+                 c->partial, c->sums, c->moments, c->frame};
   for (void* p : all) dev_free(c, p);
   std::free(c->host_coefs);
   c->host_coefs = nullptr;
@@ -326,6 +327,26 @@ void stage_release(int device, cudaStream_t stream) {
     cudaStreamSynchronize(stream);
   }
   st.in_use = false;
+}
+
+// The fp64 Box-Muller tables (abm_device.cuh, NoiseTables<double>), computed once per process in extended
+// precision (long double: 64-bit mantissa on x86-64, 113 on aarch64) and rounded to double.
+const double2* host_noise_tables() {
+  static const std::vector<double2>* tab = [] {
+    auto* t = new std::vector<double2>(NOISE_TABLE_N);
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int i = 0; i < CIRCLE_N; ++i) {
+      const long double a = two_pi * (static_cast<long double>(2 * i + 1) / (2 * CIRCLE_N));
+      (*t)[i] = make_double2(static_cast<double>(cosl(a)), static_cast<double>(sinl(a)));
+    }
+    for (int j = LOG_JMIN; j <= LOG_JMAX; ++j) {
+      const double rc = j == 0 ? 1.0 : static_cast<double>(1.0L / (1.0L + j / 128.0L));
+      // -ln of the ROUNDED reciprocal: ln m = -ln rc + log1p(m rc - 1) holds for whatever rc is
+      (*t)[CIRCLE_N + (j - LOG_JMIN)] = make_double2(rc, j == 0 ? 0.0 : static_cast<double>(-logl(static_cast<long double>(rc))));
+    }
+    return t;
+  }();
+  return tab->data();
 }
 
 template <typename Real>
@@ -434,6 +455,7 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
   a.xh = static_cast<Real*>(c->xh);
   a.coef_table = static_cast<const Coef<Real>*>(c->coef_table);
   a.tilt = static_cast<const Real*>(c->tilt_table);
+  a.noise_tables = c->noise_tables;
   a.snap = c->snap;
   a.rng_state = c->rng_state;
   a.n_traj = c->n_traj;
@@ -654,8 +676,18 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
              sizeof(double) * (N_SUMS - 1) * bps * n_param_sets) ||
       !alloc(reinterpret_cast<void**>(&c->sums), sizeof(double) * N_SUMS * n_param_sets) ||
       !alloc(reinterpret_cast<void**>(&c->moments), sizeof(MomentRec) * n_param_sets) ||
-      (c->tilt && !alloc(&c->tilt_table, c->real_size * (TILT_CHUNK + 1))))
+      (c->tilt && !alloc(&c->tilt_table, c->real_size * (TILT_CHUNK + 1))) ||
+      (c->precision == ABM_FP64 &&
+       !alloc(reinterpret_cast<void**>(&c->noise_tables), sizeof(double2) * NOISE_TABLE_N)))
     return fail(rc);
+  if (c->noise_tables) {
+    const cudaError_t e = cudaMemcpyAsync(c->noise_tables, host_noise_tables(), sizeof(double2) * NOISE_TABLE_N,
+                                          cudaMemcpyHostToDevice, c->stream);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      return fail(ABM_ECUDA);
+    }
+  }
   rc = c->precision == ABM_FP32 ? upload_coefs_and_init<float>(c, params)
                                 : upload_coefs_and_init<double>(c, params);
   if (rc != ABM_OK) return fail(rc);

@@ -256,13 +256,10 @@ __device__ __forceinline__ Normal2f box_muller_f32(uint32_t wa, uint32_t wb, flo
 // memory, which DFMA reads as an operand.
 // Valid for |t| < 2^51.
 // ---------------------------------------------------------------------------------------------
-constexpr int N_COSPI = 8, N_SINPI = 8;  // terms: degree 7 in r^2
+constexpr int N_COSPI = 8;  // terms: degree 7 in r^2
 __constant__ double C_COSPI[N_COSPI] = {
     0.9999999999999981, -4.934802200543686, 4.058712126333295, -1.3352627661817635,
     0.23533058831317874, -0.025806531975921563, 0.0019278700526981333, -0.0001004164642205389};
-__constant__ double C_SINPI[N_SINPI] = {
-    3.1415926535897927, -5.1677127800497855, 2.5501640398618677, -0.599264528825224,
-    0.08214587881631043, -0.0073703643265304155, 0.0004659870158043378, -2.113362735205297e-05};
 
 __device__ __forceinline__ double reduce_half_turns(double t, uint32_t& sign) {
   const double magic = 6755399441055744.0;  // 1.5 * 2^52: adding it rounds to an integer
@@ -282,72 +279,93 @@ __device__ __forceinline__ double cospi_f64(double t) {
   for (int k = N_COSPI - 2; k >= 0; --k) p = __fma_rn(p, r2, C_COSPI[k]);
   return flip_sign(p, sign);
 }
-// cos(pi t), sin(pi t) for t = 2 u, u = (w + 1/2) 2^-32 (the Box-Muller angle): rint(t) and the
-// remainder come from the integer w exactly -- n = (w + 2^30) >> 31, r = (int32(w - n 2^31) + 1/2) 2^-31.
-__device__ __forceinline__ void sincospi_2u_f64(uint32_t w, double* sn, double* cs) {
-  const uint32_t n = (w >> 31) + ((w >> 30) & 1u);  // = (w + 2^30) >> 31 without the overflow
-  const int32_t d = static_cast<int32_t>(w - (n << 31));
-  const uint32_t sign = n << 31;                    // parity of n -> sign bit
-  const double r = __fma_rn(static_cast<double>(d), 0x1p-31, 0x1p-32);  // exact
-  const double r2 = __dmul_rn(r, r);
-  static_assert(N_COSPI == N_SINPI, "one loop for both polynomials");
-  double p = C_COSPI[N_COSPI - 1], q = C_SINPI[N_SINPI - 1];
-#pragma unroll
-  for (int k = N_COSPI - 2; k >= 0; --k) {
-    p = __fma_rn(p, r2, C_COSPI[k]);
-    q = __fma_rn(q, r2, C_SINPI[k]);
-  }
-  *cs = flip_sign(p, sign);
-  *sn = flip_sign(__dmul_rn(q, r), sign);
+// ---------------------------------------------------------------------------------------------
+// fp64 Box-Muller from two small tables ("fp64 arithmetic").  The FP64 pipe (64 lanes/clk/SM)
+// and the FMA pipes share one dispatch port, so what this kernel is short of is FP64 operations: the
+// polynomial-only versions of round 1 took 17 (sin, cos) + 18 (-2 ln u) + 8 (sqrt) + 1 of them per pair;
+// these take 10 + 10 + 7 + 1, with function errors of the same size (<= 4e-16 absolute for sin / cos,
+// <= 3e-16 relative for ln u, < 1 ulp for the square root) against the 1e-12 trajectory tolerance.
+//
+// NoiseTables<double>: built on the host in extended precision once per process, uploaded per context,
+// copied to shared memory by every CTA of an fp64 step kernel (17.9 KB, ~1 us); the single-step path
+// reads the same shared copy, so split launches stay bit-identical.
+//   circle[i] = (cos a_i, sin a_i),  a_i = 2 pi (i + 1/2) / 1024,  i < 1024
+//   logt[t]   = (rc_j, -ln rc_j),    rc_j = fl(1 / c_j),  c_j = 1 + j / 128,  j = t + LOG_JMIN in [-37, 53]
+// ---------------------------------------------------------------------------------------------
+constexpr int CIRCLE_BITS = 10;
+constexpr int CIRCLE_N = 1 << CIRCLE_BITS;
+constexpr int LOG_JMIN = -37, LOG_JMAX = 53;
+constexpr int LOG_N = LOG_JMAX - LOG_JMIN + 1;   // 91
+constexpr int NOISE_TABLE_N = CIRCLE_N + LOG_N;  // double2 entries: circle first, then logt
+
+template <typename Real>
+struct NoiseTables {};  // fp32: none (MUFU)
+template <>
+struct NoiseTables<double> {
+  const double2* circle;
+  const double2* logt;
+};
+
+// (cos d - 1) / d^2 and sin(d) / d as linear functions of d^2 on |d| <= pi / 1024 (csrc/fit_coefficients.py:
+// 1.5e-19 and 2.8e-16 absolute on cos d, sin d), the angle scale 2 pi 2^-32, ln 2, and
+// (log1p(r) / r - 1) / r of degree 4 on |r| <= 2^-8 / 0.7109 (2.5e-16 relative to log1p r).  In constant
+// memory: a DFMA reads it as an operand.
+__constant__ double C_BMTRIG[6] = {-0.4999999999999846, 0.04166665359389469, 0.9999999999999077,
+                                   -0.16666658823003866, 1.4629180792671596e-09, 7.314590396335798e-10};
+__constant__ double C_LOG1P[6] = {-0.5, 0.3333333332925876, -0.24999999996434746, 0.20000539486857483,
+                                  -0.1666713871798388, 0.6931471805599453};
+
+// cos(2 pi u), sin(2 pi u) for u = (w + 1/2) 2^-32: the top 10 bits of w pick the table angle a_i, the low
+// 22 bits are the remainder d = 2 pi (low - 2^21 + 1/2) 2^-32, |d| <= pi / 1024, and
+// cos(a + d) = cos a + (cos a (cos d - 1) - sin a sin d),  sin(a + d) = sin a + (sin a (cos d - 1) + cos a sin d).
+__device__ __forceinline__ void sincos_2pi_u_f64(uint32_t w, const double2* __restrict__ circle, double* sn,
+                                                 double* cs) {
+  const double2 t = circle[w >> (32 - CIRCLE_BITS)];
+  const int32_t low = static_cast<int32_t>(w & ((1u << (32 - CIRCLE_BITS)) - 1u)) - (1 << (31 - CIRCLE_BITS));
+  const double d = __fma_rn(static_cast<double>(low), C_BMTRIG[4], C_BMTRIG[5]);
+  const double d2 = __dmul_rn(d, d);
+  const double cm1 = __dmul_rn(d2, __fma_rn(d2, C_BMTRIG[1], C_BMTRIG[0]));
+  const double sd = __dmul_rn(d, __fma_rn(d2, C_BMTRIG[3], C_BMTRIG[2]));
+  *cs = __fma_rn(-t.y, sd, __fma_rn(t.x, cm1, t.x));
+  *sn = __fma_rn(t.x, sd, __fma_rn(t.y, cm1, t.y));
 }
 
-// -2 ln u for u = (w + 1/2) 2^-32 = k 2^-33, k = 2w + 1, without the math library (same reason):
-// k = m 2^e with m in [sqrt(1/2), sqrt(2)) by integer surgery on the exponent field, s = (m - 1) /
-// (m + 1) by one Newton step on a single-precision reciprocal plus one residual correction,
-// ln m = 2 atanh s = s P(s^2) (|s| <= 0.1716; P a degree-6 Chebyshev fit, relative error 2.3e-16), and
-// ln u = (e - 33) ln 2 + ln m.  The sqrt(2) split keeps the two terms from cancelling as u -> 1.
-// Relative error of the whole function <= 6e-16 (fit + roundings).
-constexpr int N_ATANH2 = 7;  // terms: degree 6 in s^2
-__constant__ double C_ATANH2[N_ATANH2] = {2.0000000000000004, 0.6666666666655292, 0.40000000061741614,
-                                          0.2857141602110767, 0.22223434547517906, 0.18121934431215214,
-                                          0.16837659970680488};
-__device__ __forceinline__ float rcp_approx_f32(float x) {
-  float y;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-__device__ __forceinline__ float rsqrt_approx_f32(float x) {
-  float y;
-  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-__device__ __forceinline__ double neg2_ln_uniform_f64(uint32_t w) {
+// ln u for u = (w + 1/2) 2^-32 = k 2^-33, k = 2w + 1: k = m 2^e with m in [sqrt(1/2), sqrt(2)) by integer
+// surgery on the exponent field (the split keeps e ln 2 and ln m from cancelling as u -> 1), the table entry
+// nearest to m gives r = m / c - 1 = fma(m, rc, -1) with |r| <= 2^-8 / c, and
+// ln m = -ln rc + log1p(r),  log1p(r) = r (1 + r g(r)).  The bin around m = 1 has rc = 1 and ln rc = 0 exactly,
+// so ln u keeps its relative accuracy where it is smallest.
+__device__ __forceinline__ double ln_uniform_f64(uint32_t w, const double2* __restrict__ logt) {
   const double kd = __fma_rn(static_cast<double>(w), 2.0, 1.0);  // exact, < 2^33
   const int hi = __double2hiint(kd);
   const int mant = hi & 0x000fffff;
-  const int adj = mant >= 0x6a09f ? 1 : 0;                       // m > sqrt 2 (top 20 mantissa bits)
+  const int adj = mant >= 0x6a09f ? 1 : 0;                       // m > sqrt 2 (top 20 mantissa bits): halve it
+  // index of the nearest c_j = 1 + j / 128: m = 1.f -> j = round(128 f); m = (1.f) / 2 -> j = round(64 f) - 64
+  const int j = adj ? ((mant + 0x2000) >> 14) - 64 : (mant + 0x1000) >> 13;
   const double m = __hiloint2double(mant | ((0x3ff - adj) << 20), __double2loint(kd));
-  const double E = static_cast<double>((hi >> 20) - 1023 + adj - 33);
-  const double f = __dadd_rn(m, -1.0), g = __dadd_rn(m, 1.0);
-  double y = static_cast<double>(rcp_approx_f32(static_cast<float>(g)));
-  y = __fma_rn(y, __fma_rn(-g, y, 1.0), y);  // 2^-23 -> 2^-46; the residual step below squares it again
-  double q = __dmul_rn(f, y);
-  q = __fma_rn(__fma_rn(-g, q, f), y, q);
-  const double q2 = __dmul_rn(q, q);
-  double p = C_ATANH2[N_ATANH2 - 1];
+  const double2 t = logt[j - LOG_JMIN];
+  const double r = __fma_rn(m, t.x, -1.0);
+  double g = C_LOG1P[4];
 #pragma unroll
-  for (int j = N_ATANH2 - 2; j >= 0; --j) p = __fma_rn(p, q2, C_ATANH2[j]);
-  const double ln_u = __fma_rn(E, 0.6931471805599453, __dmul_rn(q, p));
-  return __dmul_rn(-2.0, ln_u);
+  for (int q = 3; q >= 0; --q) g = __fma_rn(g, r, C_LOG1P[q]);
+  const double p = __fma_rn(g, r, 1.0);                          // log1p(r) / r
+  const double E = static_cast<double>((hi >> 20) - 1023 + adj - 33);
+  return __fma_rn(E, C_LOG1P[5], __fma_rn(r, p, t.y));
 }
-// sqrt(a) for a normal positive a: single-precision rsqrt seed, one Newton step, one residual
-// correction (relative error <= 2.3e-16 measured).
+
+__device__ __forceinline__ double rsqrt_approx_f64(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));  // MUFU.RSQ64H: ~2^-21 from the high word of x
+  return y;
+}
+// sqrt(a) for a normal positive a: coupled Newton iteration on g -> sqrt a, h -> 1 / (2 sqrt a) from the
+// hardware seed, then one residual correction; relative error < 1 ulp (2^-21 -> 3e-13 -> rounding).
 __device__ __forceinline__ double sqrt_pos_f64(double a) {
-  double y = static_cast<double>(rsqrt_approx_f32(static_cast<float>(a)));
-  const double h = __dmul_rn(0.5, a);
-  y = __fma_rn(y, __fma_rn(-h, __dmul_rn(y, y), 0.5), y);
-  const double g = __dmul_rn(a, y);
-  return __fma_rn(__fma_rn(-g, g, a), __dmul_rn(0.5, y), g);
+  const double y = rsqrt_approx_f64(a);
+  const double g0 = __dmul_rn(a, y), h0 = __dmul_rn(0.5, y);
+  const double r0 = __fma_rn(-g0, h0, 0.5);
+  const double g1 = __fma_rn(g0, r0, g0), h1 = __fma_rn(h0, r0, h0);
+  return __fma_rn(__fma_rn(-g1, g1, a), h1, g1);
 }
 
 struct Normal2d {
@@ -359,10 +377,11 @@ __device__ __forceinline__ double uniform_f64(uint32_t w) {
   return __fma_rn(static_cast<double>(w), 0x1p-32, 0x1p-33);  // (w + 0.5) 2^-32, exact
 }
 
-__device__ __forceinline__ Normal2d box_muller_f64(uint32_t wa, uint32_t wb, double sigma) {
+__device__ __forceinline__ Normal2d box_muller_f64(uint32_t wa, uint32_t wb, double sigma,
+                                                   const NoiseTables<double>& nt) {
   Normal2d o;
-  o.rho = __dmul_rn(sigma, sqrt_pos_f64(neg2_ln_uniform_f64(wa)));
-  sincospi_2u_f64(wb, &o.sn, &o.cs);
+  o.rho = __dmul_rn(sigma, sqrt_pos_f64(__dmul_rn(-2.0, ln_uniform_f64(wa, nt.logt))));
+  sincos_2pi_u_f64(wb, nt.circle, &o.sn, &o.cs);
   return o;
 }
 

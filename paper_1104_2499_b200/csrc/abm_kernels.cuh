@@ -79,6 +79,7 @@ struct StepArgs {
   uint32_t traj_hi;              // high word of every global trajectory index, if shared
   uint32_t traj_hi_shared;       // 1: all trajectories of the launch share traj_hi
   uint32_t rk0[10], rk1[10];     // Philox round keys k0 + r W0, k1 + r W1 (host-computed: constant-bank operands)
+  const double2* noise_tables;   // fp64: circle and log tables of the Box-Muller transform (NoiseTables), else nullptr
   Coef<Real> coef0;              // the single set's coefficients (used when UNIFORM)
 };
 
@@ -218,7 +219,7 @@ template <>
 struct Noise4<float> {
   static constexpr float SIGN = Normal2f::NEGATED ? -1.0f : 1.0f;
   Normal2f a, b;
-  __device__ __forceinline__ Noise4(const uint4& w, const Coef<float>& k)
+  __device__ __forceinline__ Noise4(const uint4& w, const Coef<float>& k, const NoiseTables<float>& = {})
       : a(box_muller_f32(w.x, w.y, k.s2, k.bm_o)), b(box_muller_f32(w.z, w.w, k.s2, k.bm_o)) {}
   __device__ __forceinline__ Noise4(const Normal2f& a_, const Normal2f& b_) : a(a_), b(b_) {}
 };
@@ -226,8 +227,8 @@ template <>
 struct Noise4<double> {
   static constexpr double SIGN = Normal2d::NEGATED ? -1.0 : 1.0;
   Normal2d a, b;
-  __device__ __forceinline__ Noise4(const uint4& w, const Coef<double>& k)
-      : a(box_muller_f64(w.x, w.y, k.s2)), b(box_muller_f64(w.z, w.w, k.s2)) {}
+  __device__ __forceinline__ Noise4(const uint4& w, const Coef<double>& k, const NoiseTables<double>& nt)
+      : a(box_muller_f64(w.x, w.y, k.s2, nt)), b(box_muller_f64(w.z, w.w, k.s2, nt)) {}
 };
 
 template <typename Real, int INTEG, int TILT, bool PRECISE>
@@ -264,8 +265,8 @@ __device__ __forceinline__ void four_steps_z(State<Real>& s, const Coef<Real>& c
 // Four steps from one Philox block.
 template <typename Real, int INTEG, int TILT, bool PRECISE>
 __device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf, const uint4& w,
-                                           const Real*& tl) {
-  const Noise4<Real> z(w, cf);
+                                           const Real*& tl, const NoiseTables<Real>& nt) {
+  const Noise4<Real> z(w, cf, nt);
   four_steps_z<Real, INTEG, TILT, PRECISE>(s, cf, z, tl);
 }
 
@@ -324,16 +325,19 @@ struct Integrate {
   State<Real>& s;
   const uint64_t k;
   const bool active;
+  const NoiseTables<Real> nt;
   const Real* tl;
   __device__ __forceinline__ Integrate(const StepArgs<Real>& a_, const Coef<Real>& cf_, State<Real>& s_,
-                                       uint64_t k_, bool active_)
-      : a(a_), cf(cf_), s(s_), k(k_), active(active_), tl(nullptr) {}
+                                       uint64_t k_, bool active_, const NoiseTables<Real>& nt_)
+      : a(a_), cf(cf_), s(s_), k(k_), active(active_), nt(nt_), tl(nullptr) {}
   // a run of whole blocks starts at step n
   __device__ __forceinline__ void start(uint64_t n) { tl = TILT ? a.tilt + (n - a.tilt_base) : nullptr; }
-  __device__ __forceinline__ void block(const uint4& w) { four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl); }
+  __device__ __forceinline__ void block(const uint4& w) {
+    four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl, nt);
+  }
   // step n alone; w holds the words of its pair where the block layout has them
   __device__ __forceinline__ void single(const uint4& w, uint64_t n) {
-    const Noise4<Real> z(w, cf);
+    const Noise4<Real> z(w, cf, nt);
     const bool second = (n >> 1) & 1u;
     const Real rho = Noise4<Real>::SIGN * (second ? z.b.rho : z.a.rho);
     const Real cs = (n & 1u) ? (second ? z.b.sn : z.a.sn) : (second ? z.b.cs : z.a.cs);
@@ -544,6 +548,15 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint32_
 #define ABM_PHILOX_TABLE 1
 #endif
 
+// fp64: every CTA copies the Box-Muller tables (17.9 KB) from global to shared memory once per launch.
+__device__ __forceinline__ NoiseTables<float> stage_noise_tables(const StepArgs<float>&) { return {}; }
+__device__ __forceinline__ NoiseTables<double> stage_noise_tables(const StepArgs<double>& a) {
+  __shared__ double2 tabs[NOISE_TABLE_N];
+  for (int i = threadIdx.x; i < NOISE_TABLE_N; i += STEP_BLOCK) tabs[i] = a.noise_tables[i];
+  __syncthreads();
+  return {tabs, tabs + CIRCLE_N};
+}
+
 template <typename Real, int INTEG, bool TILT, int COEF, bool PRECISE, bool XS>
 __global__ void __launch_bounds__(STEP_BLOCK, step_min_blocks<Real, INTEG, COEF>())
 step_kernel(const __grid_constant__ StepArgs<Real> a) {
@@ -585,7 +598,7 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
   // straddles a multiple of 2^32); the block-head table of run_steps needs that.
   uint4 S = make_uint4(0u, 0u, 0u, 0u);
   constexpr int TL = TILT ? (UNIFORM ? 2 : 1) : 0;  // what the tilt table holds (one_step)
-  Integrate<Real, INTEG, TL, PRECISE> body(a, cf, s, k, active);
+  Integrate<Real, INTEG, TL, PRECISE> body(a, cf, s, k, active, stage_noise_tables(a));
   if (XS) {
     S = a.rng_state[k];
     run_steps<Real, false, true>(a, 0u, 0u, body, S);
