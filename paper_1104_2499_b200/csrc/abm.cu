@@ -339,10 +339,13 @@ const double2* host_noise_tables() {
       const long double a = two_pi * (static_cast<long double>(2 * i + 1) / (2 * CIRCLE_N));
       (*t)[i] = make_double2(static_cast<double>(cosl(a)), static_cast<double>(sinl(a)));
     }
-    for (int j = LOG_JMIN; j <= LOG_JMAX; ++j) {
-      const double rc = j == 0 ? 1.0 : static_cast<double>(1.0L / (1.0L + j / 128.0L));
+    const long double ln2 = 0.693147180559945309417232121458176568L;
+    for (int i = 0; i < LOG_N; ++i) {
       // -ln of the ROUNDED reciprocal: ln m = -ln rc + log1p(m rc - 1) holds for whatever rc is
-      (*t)[CIRCLE_N + (j - LOG_JMIN)] = make_double2(rc, j == 0 ? 0.0 : static_cast<double>(-logl(static_cast<long double>(rc))));
+      const double rc = static_cast<double>(1.0L / (1.0L + i / 256.0L));
+      long double lnc = -logl(static_cast<long double>(rc));
+      if (i >= LOG_ADJ_FROM) lnc -= ln2;
+      (*t)[CIRCLE_N + i] = make_double2(rc, (i == 0 || i == LOG_N - 1) ? 0.0 : static_cast<double>(lnc));
     }
     return t;
   }();

@@ -283,19 +283,19 @@ __device__ __forceinline__ double cospi_f64(double t) {
 // fp64 Box-Muller from two small tables ("fp64 arithmetic").  The FP64 pipe (64 lanes/clk/SM)
 // and the FMA pipes share one dispatch port, so what this kernel is short of is FP64 operations: the
 // polynomial-only versions of round 1 took 17 (sin, cos) + 18 (-2 ln u) + 8 (sqrt) + 1 of them per pair;
-// these take 10 + 10 + 7 + 1, with function errors of the same size (<= 4e-16 absolute for sin / cos,
-// <= 3e-16 relative for ln u, < 1 ulp for the square root) against the 1e-12 trajectory tolerance.
+// these take 10 + 9 + 7 + 1, with function errors of the same size (<= 4e-16 absolute for sin / cos,
+// <= 7e-16 relative for ln u, < 1 ulp for the square root) against the 1e-12 trajectory tolerance.
 //
 // NoiseTables<double>: built on the host in extended precision once per process, uploaded per context,
-// copied to shared memory by every CTA of an fp64 step kernel (17.9 KB, ~1 us); the single-step path
+// copied to shared memory by every CTA of an fp64 step kernel (20.5 KB, ~1 us); the single-step path
 // reads the same shared copy, so split launches stay bit-identical.
 //   circle[i] = (cos a_i, sin a_i),  a_i = 2 pi (i + 1/2) / 1024,  i < 1024
-//   logt[t]   = (rc_j, -ln rc_j),    rc_j = fl(1 / c_j),  c_j = 1 + j / 128,  j = t + LOG_JMIN in [-37, 53]
+//   logt[i]   = (rc_i, -ln rc_i - [i >= LOG_ADJ_FROM] ln 2),  rc_i = fl(1 / c_i),  c_i = 1 + i / 256,  i <= 256
 // ---------------------------------------------------------------------------------------------
 constexpr int CIRCLE_BITS = 10;
 constexpr int CIRCLE_N = 1 << CIRCLE_BITS;
-constexpr int LOG_JMIN = -37, LOG_JMAX = 53;
-constexpr int LOG_N = LOG_JMAX - LOG_JMIN + 1;   // 91
+constexpr int LOG_N = 257;
+constexpr int LOG_ADJ_FROM = 106;                // c_i >= 1.412 ~ sqrt 2: the mantissa is taken as m / 2
 constexpr int NOISE_TABLE_N = CIRCLE_N + LOG_N;  // double2 entries: circle first, then logt
 
 template <typename Real>
@@ -307,13 +307,13 @@ struct NoiseTables<double> {
 };
 
 // (cos d - 1) / d^2 and sin(d) / d as linear functions of d^2 on |d| <= pi / 1024 (csrc/fit_coefficients.py:
-// 1.5e-19 and 2.8e-16 absolute on cos d, sin d), the angle scale 2 pi 2^-32, ln 2, and
-// (log1p(r) / r - 1) / r of degree 4 on |r| <= 2^-8 / 0.7109 (2.5e-16 relative to log1p r).  In constant
-// memory: a DFMA reads it as an operand.
+// 1.5e-19 and 2.8e-16 absolute on cos d, sin d), the angle scale C = 2 pi 2^-32 and (1/2 - 2^21) C, and
+// (log1p(r) / r - 1) / r of degree 3 on |r| <= 2^-9 (6e-16 relative to log1p r), ln 2 and 2.  In constant
+// memory: a DFMA reads it as an operand (a 64-bit literal costs two moves per use).
 __constant__ double C_BMTRIG[6] = {-0.4999999999999846, 0.04166665359389469, 0.9999999999999077,
-                                   -0.16666658823003866, 1.4629180792671596e-09, 7.314590396335798e-10};
-__constant__ double C_LOG1P[6] = {-0.5, 0.3333333332925876, -0.24999999996434746, 0.20000539486857483,
-                                  -0.1666713871798388, 0.6931471805599453};
+                                   -0.16666658823003866, 1.4629180792671596e-09, -0.0030679608443122427};
+__constant__ double C_LOG1P[6] = {-0.49999999999969563, 0.33333333333307247, -0.2500006370268452,
+                                  0.20000054602306092, 0.6931471805599453, 2.0};
 
 // cos(2 pi u), sin(2 pi u) for u = (w + 1/2) 2^-32: the top 10 bits of w pick the table angle a_i, the low
 // 22 bits are the remainder d = 2 pi (low - 2^21 + 1/2) 2^-32, |d| <= pi / 1024, and
@@ -321,7 +321,7 @@ __constant__ double C_LOG1P[6] = {-0.5, 0.3333333332925876, -0.24999999996434746
 __device__ __forceinline__ void sincos_2pi_u_f64(uint32_t w, const double2* __restrict__ circle, double* sn,
                                                  double* cs) {
   const double2 t = circle[w >> (32 - CIRCLE_BITS)];
-  const int32_t low = static_cast<int32_t>(w & ((1u << (32 - CIRCLE_BITS)) - 1u)) - (1 << (31 - CIRCLE_BITS));
+  const uint32_t low = w & ((1u << (32 - CIRCLE_BITS)) - 1u);
   const double d = __fma_rn(static_cast<double>(low), C_BMTRIG[4], C_BMTRIG[5]);
   const double d2 = __dmul_rn(d, d);
   const double cm1 = __dmul_rn(d2, __fma_rn(d2, C_BMTRIG[1], C_BMTRIG[0]));
@@ -330,27 +330,25 @@ __device__ __forceinline__ void sincos_2pi_u_f64(uint32_t w, const double2* __re
   *sn = __fma_rn(t.x, sd, __fma_rn(t.y, cm1, t.y));
 }
 
-// ln u for u = (w + 1/2) 2^-32 = k 2^-33, k = 2w + 1: k = m 2^e with m in [sqrt(1/2), sqrt(2)) by integer
-// surgery on the exponent field (the split keeps e ln 2 and ln m from cancelling as u -> 1), the table entry
-// nearest to m gives r = m / c - 1 = fma(m, rc, -1) with |r| <= 2^-8 / c, and
-// ln m = -ln rc + log1p(r),  log1p(r) = r (1 + r g(r)).  The bin around m = 1 has rc = 1 and ln rc = 0 exactly,
-// so ln u keeps its relative accuracy where it is smallest.
+// ln u for u = (w + 1/2) 2^-32 = k 2^-33, k = 2w + 1 = m 2^e, m in [1, 2): the table entry nearest to m gives
+// r = m / c - 1 = fma(m, rc, -1), |r| <= 2^-9, and ln m = -ln rc + log1p(r), log1p(r) = r (1 + r g(r)).
+// For c >= 1.412 the entry holds -ln rc - ln 2 and e counts one more (m taken as m / 2 in [0.706, 1)), so
+// that e ln 2 and ln m never cancel as u -> 1; the last entry, c = 2, has rc = 1/2 and 0 exactly, and
+// ln u keeps its relative accuracy where it is smallest.
 __device__ __forceinline__ double ln_uniform_f64(uint32_t w, const double2* __restrict__ logt) {
-  const double kd = __fma_rn(static_cast<double>(w), 2.0, 1.0);  // exact, < 2^33
+  const double kd = __fma_rn(static_cast<double>(w), C_LOG1P[5], 1.0);  // exact, < 2^33
   const int hi = __double2hiint(kd);
   const int mant = hi & 0x000fffff;
-  const int adj = mant >= 0x6a09f ? 1 : 0;                       // m > sqrt 2 (top 20 mantissa bits): halve it
-  // index of the nearest c_j = 1 + j / 128: m = 1.f -> j = round(128 f); m = (1.f) / 2 -> j = round(64 f) - 64
-  const int j = adj ? ((mant + 0x2000) >> 14) - 64 : (mant + 0x1000) >> 13;
-  const double m = __hiloint2double(mant | ((0x3ff - adj) << 20), __double2loint(kd));
-  const double2 t = logt[j - LOG_JMIN];
+  const int i = (mant + 0x800) >> 12;                                   // round(256 (m - 1)), 0 .. 256
+  const double m = __hiloint2double(mant | 0x3ff00000, __double2loint(kd));
+  const double2 t = logt[i];
   const double r = __fma_rn(m, t.x, -1.0);
-  double g = C_LOG1P[4];
+  double g = C_LOG1P[3];
 #pragma unroll
-  for (int q = 3; q >= 0; --q) g = __fma_rn(g, r, C_LOG1P[q]);
-  const double p = __fma_rn(g, r, 1.0);                          // log1p(r) / r
-  const double E = static_cast<double>((hi >> 20) - 1023 + adj - 33);
-  return __fma_rn(E, C_LOG1P[5], __fma_rn(r, p, t.y));
+  for (int q = 2; q >= 0; --q) g = __fma_rn(g, r, C_LOG1P[q]);
+  const double p = __fma_rn(g, r, 1.0);                                 // log1p(r) / r
+  const double E = static_cast<double>((hi >> 20) - (1023 + 33) + (i >= LOG_ADJ_FROM ? 1 : 0));
+  return __fma_rn(E, C_LOG1P[4], __fma_rn(r, p, t.y));
 }
 
 __device__ __forceinline__ double rsqrt_approx_f64(double x) {

@@ -299,6 +299,9 @@ constexpr int PHILOX_CHUNK = STEP_BLOCK;  // table entries per refill = threads 
 #ifndef ABM_UNROLL2
 #define ABM_UNROLL2 1
 #endif
+#ifndef ABM_UNROLL2_F64
+#define ABM_UNROLL2_F64 1
+#endif
 #ifndef ABM_RK_CONST
 #define ABM_RK_CONST 1
 #endif
@@ -405,7 +408,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint32_
           const uint32_t seg = left < to_snap ? left : static_cast<uint32_t>(to_snap);  // >= 1
           const bool last = seg == left;
           uint32_t ahead = last ? seg - 1u : seg;  // blocks of this segment with a look-ahead draw
-          if constexpr (sizeof(Real) == 4 && ABM_UNROLL2 != 0) {  // two blocks per trip, as for Philox
+          if constexpr ((sizeof(Real) == 4 || ABM_UNROLL2_F64 != 0) && ABM_UNROLL2 != 0) {  // two blocks per trip, as for Philox
             if (ahead & 1u) {
               const uint4 w_next = xorshift128_x4(S);
               body.block(w);
@@ -459,7 +462,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint32_
             // fp32: two blocks per loop trip -- the look-ahead words alternate between two register
             // sets, so no moves rotate them and the loop overhead is halved (fp64 is short of
             // registers: one block per trip).
-            if constexpr (sizeof(Real) == 4 && ABM_UNROLL2 != 0) {
+            if constexpr ((sizeof(Real) == 4 || ABM_UNROLL2_F64 != 0) && ABM_UNROLL2 != 0) {
               if (seg & 1u) {
                 const uint4 u = *tp++;
                 const uint4 w_next = PHILOX_FINISH(pt, u, a, k0, k1);
@@ -633,6 +636,10 @@ step_kernel(const __grid_constant__ StepArgs<Real> a) {
 // ---------------------------------------------------------------------------------------------
 constexpr int SMALL_CHUNK = 16;    // Philox blocks per chunk (64 steps)
 constexpr int SMALL_TRAJ = 32;     // trajectories per CTA (one integrating warp)
+#ifndef ABM_SMALL_UNROLL
+#define ABM_SMALL_UNROLL 4
+#endif
+constexpr int SMALL_UNROLL = ABM_SMALL_UNROLL;  // Philox blocks per trip of the integrating warp's loop
 #ifndef ABM_SMALL_PRODUCERS
 #define ABM_SMALL_PRODUCERS 3
 #endif
@@ -688,7 +695,7 @@ step_kernel_small(const __grid_constant__ StepArgs<float> a) {
     if (warp == 0) {
       const uint32_t first = c * SMALL_CHUNK;
       const uint32_t cnt = n_blocks - first < SMALL_CHUNK ? n_blocks - first : SMALL_CHUNK;
-#pragma unroll 1
+#pragma unroll SMALL_UNROLL
       for (uint32_t j = 0; j < cnt; ++j) {
         float(*slot)[SMALL_TRAJ] = ring[buf][j];
         Normal2f za, zb;

@@ -5,7 +5,7 @@
 Near-minimax fits by interpolation at Chebyshev nodes, computed with mpmath at 60 digits, rounded to
 double; the printed errors are those of the ROUNDED coefficients in exact arithmetic.
   C_COSPI    cos(pi r) as a polynomial in r^2, |r| <= 1/2                (force, fp64: cospi_f64)
-  C_LOG1P    (log1p(r)/r - 1)/r, |r| <= 2^-8 / 0.7109375                 (Box-Muller, fp64: table-driven log)
+  C_LOG1P    (log1p(r)/r - 1)/r, |r| <= 2^-9                             (Box-Muller, fp64: table-driven log)
   C_BMTRIG   (cos d - 1)/d^2 and sin(d)/d in d^2, |d| <= pi/1024         (Box-Muller, fp64: circle table)
 """
 import mpmath as mp
@@ -47,9 +47,9 @@ if __name__ == "__main__":
     c = cheb_fit(f, mp.mpf(0), quarter, 7)
     show("C_COSPI", c, max_err(f, c, mp.mpf(0), quarter), "max abs error")
 
-    R = mp.mpf(2)**-8 / mp.mpf("0.7109375") + mp.mpf(2)**-19
+    R = mp.mpf(2)**-9 * (1 + mp.mpf(2)**-10)
     g = lambda r: mp.mpf(-1) / 2 + r / 3 if abs(r) < mp.mpf(10)**-25 else (mp.log1p(r) / r - 1) / r
-    c = cheb_fit(g, -R, R, 4)
+    c = cheb_fit(g, -R, R, 3)
     # error of log1p(r) = r (1 + r g(r)) relative to log1p(r)
     show("C_LOG1P", c, max_err(g, c, -R, R, lambda r: r * r / abs(mp.log1p(r)) if r != 0 else 0),
          "max error relative to log1p(r)")

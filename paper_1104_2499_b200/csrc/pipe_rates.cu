@@ -36,7 +36,7 @@ enum Op {
 static const char* OP_NAME[N_OPS] = {
   "FFMA r,r,r", "FFMA r,r,c[]", "FFMA r,imm,r", "FMUL r,r", "FADD r,r", "IMAD.LO r,r,r",
   "IMAD.WIDE.U32 r,r", "IMAD.WIDE r,imm + LOP3", "LOP3 (xor3)", "IADD3 r,r,r", "SHF.R",
-  "FMUL+MUFU.COS", "FMUL+MUFU.SIN", "MUFU.LG2", "MUFU.SQRT", "MUFU.RSQ", "MUFU.EX2", "MUFU.RCP",
+  "FMUL+MUFU.COS", "FMUL+MUFU.SIN", "MUFU.LG2", "MUFU.SQRT", "MUFU.RSQ", "MUFU.EX2", "FADD+MUFU.RCP",
   "DFMA", "DMUL", "DADD", "I2F.U32", "F2I.U32", "FFMA2 (f32x2, per elem)", "FRND"};
 
 struct Regs {
@@ -78,7 +78,9 @@ __device__ __forceinline__ void one(Regs& r, int j, float fb, float fc, uint32_t
   if (OP == MUFU_SQRT) asm volatile("sqrt.approx.ftz.f32 %0, %0;" : "+f"(r.f[j]));
   if (OP == MUFU_RSQ) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(r.f[j]));
   if (OP == MUFU_EX2) asm volatile("ex2.approx.ftz.f32 %0, %0;" : "+f"(r.f[j]));
-  if (OP == MUFU_RCP) asm volatile("rcp.approx.ftz.f32 %0, %0;" : "+f"(r.f[j]));
+  // with an FADD in the chain: ptxas folds rcp(rcp(x)) to x even in volatile asm, which emptied the loop
+  if (OP == MUFU_RCP)
+    asm volatile("{\n\t.reg .f32 t;\n\trcp.approx.ftz.f32 t, %0;\n\tadd.rn.f32 %0, t, %1;\n\t}" : "+f"(r.f[j]) : "f"(fc));
   if (OP == DFMA_) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(r.d[j]) : "d"(db), "d"(dc));
   if (OP == DMUL_) asm volatile("mul.rn.f64 %0, %0, %1;" : "+d"(r.d[j]) : "d"(db));
   if (OP == DADD_) asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(r.d[j]) : "d"(dc));
@@ -182,11 +184,12 @@ double run(const Dev& d, int threads, int ctas_per_sm, int iters) {
 
 template <int OP>
 void single(const Dev& d) {
+  const double r4 = run<OP, N_OPS>(d, 128, 1, 2000);    // 1 warp / scheduler: what ONE warp can issue
   const double r8 = run<OP, N_OPS>(d, 256, 1, 2000);    // 2 warps / scheduler
   const double r16 = run<OP, N_OPS>(d, 512, 1, 2000);   // 4 warps / scheduler
   const double r32 = run<OP, N_OPS>(d, 1024, 1, 1000);  // 8 warps / scheduler
   const double w = OP == FFMA2_ ? 2.0 : 1.0;  // two fp32 FMAs per FFMA2
-  std::printf("%-22s %8.1f %8.1f %8.1f\n", OP_NAME[OP], w * r8, w * r16, w * r32);
+  std::printf("%-22s %8.1f %8.1f %8.1f %8.1f\n", OP_NAME[OP], w * r4, w * r8, w * r16, w * r32);
 }
 
 template <int OPA, int OPB>
@@ -197,6 +200,13 @@ void mix(const Dev& d) {
               (wa + wb) * r);
 }
 
+template <int OPA, int OPB>
+void mix1(const Dev& d) {
+  const double r = run<OPA, OPB>(d, 128, 1, 2000);
+  const double wa = OPA == FFMA2_ ? 2.0 : 1.0, wb = OPB == FFMA2_ ? 2.0 : 1.0;
+  std::printf("%-24s + %-24s %8.1f / %8.1f, %8.1f total\n", OP_NAME[OPA], OP_NAME[OPB], wa * r, wb * r,
+              (wa + wb) * r);
+}
 
 // ---------------------------------------------------------------------------------------------
 // Third table: the instruction mix of the fp32 Euler-Maruyama step loop (one Philox block = four
@@ -290,6 +300,240 @@ void loop_mix_row(const Dev& d, const char* name) {
               loop_mix<MODE>(d, 12));
 }
 
+// ---------------------------------------------------------------------------------------------
+// Fourth table: the fp32 Heun + tilt loop (config[3]) as independent chains, per Philox block = four steps:
+// 120 FFMA/FADD/FMUL, 10 x (FMUL.RZ + MUFU.COS) + 6 more MUFU, 16 x (IMAD.WIDE + LOP3), 4 LDG + 1 LDS.128,
+// F2I + I2F, 14 more ALU instructions.  MODE bits: 1 FP32, 2 Philox, 4 MUFU, 8 ALU extras, 16 loads + conversions.
+// ---------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(128) heun_mix_kernel(int iters, const float* __restrict__ in,
+                                                       float* __restrict__ out,
+                                                       long long* __restrict__ cycles) {
+  __shared__ float4 sh[128];
+  float f[12], m[8];
+  uint32_t u[8];
+  const float fb = in[0], fc = in[1];
+  const uint32_t ub = __float_as_uint(in[2]) | 1u, uc = __float_as_uint(in[3]);
+#pragma unroll
+  for (int j = 0; j < 12; ++j) f[j] = in[4] + j + threadIdx.x;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    u[j] = ub * (j + 3) + threadIdx.x;
+    m[j] = in[5] + j * 0.1f;
+  }
+  sh[threadIdx.x] = make_float4(fb, fc, fb, fc);
+  __syncthreads();
+  const float* g = in;
+  float ld = 0.f;
+  const long long t0 = clock64();
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {  // half a block per pass: 60 FP32, 8 IW, 5 cos + 3 MUFU, 7 ALU, 2 LDG
+      if (MODE & 1) { PR_FF(f[0]) PR_FF(f[1]) PR_FF(f[2]) PR_FF(f[3]) PR_FF(f[4]) PR_FF(f[5]) }
+      if (MODE & 2) { PR_IW(u[0]) PR_IW(u[1]) }
+      if (MODE & 4) { PR_MC(m[0]) PR_MC(m[1]) }
+      if (MODE & 16) { float t; asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(t) : "l"(g + (it & 3))); ld += t; }
+      if (MODE & 1) { PR_FF(f[6]) PR_FF(f[7]) PR_FF(f[8]) PR_FF(f[9]) PR_FF(f[10]) PR_FF(f[11]) PR_FF(f[0]) PR_FF(f[1]) }
+      if (MODE & 2) { PR_IW(u[2]) PR_IW(u[3]) }
+      if (MODE & 4) { PR_MC(m[2]) PR_ML(m[3]) }
+      if (MODE & 8) { PR_LX(u[4]) PR_LX(u[5]) PR_LX(u[6]) }
+      if (MODE & 1) { PR_FF(f[2]) PR_FF(f[3]) PR_FF(f[4]) PR_FF(f[5]) PR_FF(f[6]) PR_FF(f[7]) PR_FF(f[8]) PR_FF(f[9]) }
+      if (MODE & 2) { PR_IW(u[0]) PR_IW(u[1]) }
+      if (MODE & 4) { PR_MC(m[4]) PR_MS(m[5]) }
+      if (MODE & 16) { float t; asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(t) : "l"(g + ((it + 1) & 3))); ld += t; }
+      if (MODE & 1) { PR_FF(f[10]) PR_FF(f[11]) PR_FF(f[0]) PR_FF(f[1]) PR_FF(f[2]) PR_FF(f[3]) PR_FF(f[4]) PR_FF(f[5]) }
+      if (MODE & 2) { PR_IW(u[2]) PR_IW(u[3]) }
+      if (MODE & 4) { PR_MC(m[6]) PR_ME(m[7]) }
+      if (MODE & 8) { PR_LX(u[7]) PR_LX(u[4]) PR_LX(u[5]) PR_LX(u[6]) }
+      if (MODE & 1) {
+        PR_FF(f[6]) PR_FF(f[7]) PR_FF(f[8]) PR_FF(f[9]) PR_FF(f[10]) PR_FF(f[11]) PR_FF(f[0]) PR_FF(f[1]) PR_FF(f[2]) PR_FF(f[3])
+        PR_FF(f[4]) PR_FF(f[5]) PR_FF(f[6]) PR_FF(f[7]) PR_FF(f[8]) PR_FF(f[9]) PR_FF(f[10]) PR_FF(f[11]) PR_FF(f[0]) PR_FF(f[1])
+        PR_FF(f[2]) PR_FF(f[3]) PR_FF(f[4]) PR_FF(f[5]) PR_FF(f[6]) PR_FF(f[7]) PR_FF(f[8]) PR_FF(f[9]) PR_FF(f[10]) PR_FF(f[11])
+      }
+    }
+    if (MODE & 16) {  // once per block: the block-head LDS.128 and the fold's F2I + I2F
+      const float4 t = sh[(threadIdx.x + it) & 127];
+      ld += t.x;
+      asm volatile("{\n\t.reg .s32 t;\n\tcvt.rni.s32.f32 t, %0;\n\tcvt.rn.f32.s32 %0, t;\n\t}" : "+f"(m[7]));
+    }
+  }
+  const long long t1 = clock64();
+  float acc = ld;
+  uint32_t ua = 0;
+#pragma unroll
+  for (int j = 0; j < 12; ++j) acc += f[j];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    ua ^= u[j];
+    acc += m[j];
+  }
+  if (static_cast<double>(acc) + static_cast<double>(ua) == 12345.0) out[threadIdx.x] = acc;
+  if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fifth table: the fp64 Euler-Maruyama loop (config[4]) as independent chains, per Philox block:
+// 114 DFMA + 22 DMUL + 12 DADD, 16 x (IMAD.WIDE + LOP3), 6 I2F.F64 + 2 MUFU.RSQ64H, 19 integer moves /
+// multiplies on the FMA pipe (IMAD.MOV, IMAD.U32), 41 ALU-pipe instructions, 5 LDS.128.
+// MODE bits: 1 FP64, 2 Philox, 4 conversions + MUFU, 8 ALU, 16 FMA-pipe integer, 32 LDS.
+// ---------------------------------------------------------------------------------------------
+#define PR_DF(r) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(r) : "d"(db), "d"(dc));
+#define PR_DM(r) asm volatile("mul.rn.f64 %0, %0, %1;" : "+d"(r) : "d"(db));
+#define PR_DA(r) asm volatile("add.rn.f64 %0, %0, %1;" : "+d"(r) : "d"(dc));
+#define PR_IM(r) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(r) : "r"(ub), "r"(uc));
+#define PR_ID(r, x) asm volatile("cvt.rn.f64.s32 %0, %1;" : "=d"(r) : "r"(x));
+#define PR_RS(r) asm volatile("rsqrt.approx.ftz.f64 %0, %0;" : "+d"(r));
+
+template <int MODE>
+__global__ void __launch_bounds__(128) f64_mix_kernel(int iters, const float* __restrict__ in,
+                                                      float* __restrict__ out,
+                                                      long long* __restrict__ cycles) {
+  __shared__ double2 sh[128];
+  double d[12], cv[3], rs = 1.5;
+  uint32_t u[8];
+  const double db = static_cast<double>(in[0]), dc = static_cast<double>(in[1]);
+  const uint32_t ub = __float_as_uint(in[2]) | 1u, uc = __float_as_uint(in[3]);
+#pragma unroll
+  for (int j = 0; j < 12; ++j) d[j] = static_cast<double>(in[4]) + j + threadIdx.x;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) u[j] = ub * (j + 3) + threadIdx.x;
+  cv[0] = cv[1] = cv[2] = 0;
+  sh[threadIdx.x] = make_double2(db, dc);
+  __syncthreads();
+  double ld = 0;
+  const long long t0 = clock64();
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {  // half a block: 57 DFMA, 11 DMUL, 6 DADD, 8 IW, 3 I2F, 1 RSQ, 20 ALU, 10 IMAD
+      if (MODE & 1) { PR_DF(d[0]) PR_DF(d[1]) PR_DF(d[2]) PR_DF(d[3]) PR_DM(d[4]) PR_DF(d[5]) PR_DF(d[6]) PR_DA(d[7]) }
+      if (MODE & 2) { PR_IW(u[0]) PR_IW(u[1]) }
+      if (MODE & 4) { PR_ID(cv[0], u[4]) }
+      if (MODE & 8) { PR_LX(u[4]) PR_LX(u[5]) PR_LX(u[6]) PR_LX(u[7]) PR_LX(u[4]) }
+      if (MODE & 16) { PR_IM(u[5]) PR_IM(u[6]) PR_IM(u[7]) }
+      if (MODE & 1) { PR_DF(d[8]) PR_DF(d[9]) PR_DF(d[10]) PR_DM(d[11]) PR_DF(d[0]) PR_DF(d[1]) PR_DF(d[2]) PR_DF(d[3]) PR_DM(d[4]) PR_DA(d[5]) }
+      if (MODE & 2) { PR_IW(u[2]) PR_IW(u[3]) }
+      if (MODE & 32) { const double2 t = sh[(threadIdx.x + it + q) & 127]; ld += t.x; }
+      if (MODE & 8) { PR_LX(u[5]) PR_LX(u[6]) PR_LX(u[7]) PR_LX(u[4]) PR_LX(u[5]) }
+      if (MODE & 1) { PR_DF(d[6]) PR_DF(d[7]) PR_DF(d[8]) PR_DF(d[9]) PR_DM(d[10]) PR_DF(d[11]) PR_DF(d[0]) PR_DF(d[1]) PR_DM(d[2]) PR_DA(d[3]) }
+      if (MODE & 4) { PR_ID(cv[1], u[5]) PR_RS(rs) }
+      if (MODE & 16) { PR_IM(u[4]) PR_IM(u[5]) PR_IM(u[6]) }
+      if (MODE & 2) { PR_IW(u[0]) PR_IW(u[1]) }
+      if (MODE & 1) { PR_DF(d[4]) PR_DF(d[5]) PR_DF(d[6]) PR_DF(d[7]) PR_DM(d[8]) PR_DF(d[9]) PR_DF(d[10]) PR_DF(d[11]) PR_DM(d[0]) PR_DA(d[1]) }
+      if (MODE & 8) { PR_LX(u[6]) PR_LX(u[7]) PR_LX(u[4]) PR_LX(u[5]) PR_LX(u[6]) }
+      if (MODE & 32) { const double2 t = sh[(threadIdx.x + 2 * it + q) & 127]; ld += t.y; }
+      if (MODE & 1) { PR_DF(d[2]) PR_DF(d[3]) PR_DF(d[4]) PR_DF(d[5]) PR_DM(d[6]) PR_DF(d[7]) PR_DF(d[8]) PR_DF(d[9]) PR_DM(d[10]) PR_DA(d[11]) }
+      if (MODE & 2) { PR_IW(u[2]) PR_IW(u[3]) }
+      if (MODE & 4) { PR_ID(cv[2], u[6]) }
+      if (MODE & 16) { PR_IM(u[7]) PR_IM(u[4]) PR_IM(u[5]) PR_IM(u[6]) }
+      if (MODE & 8) { PR_LX(u[7]) PR_LX(u[4]) PR_LX(u[5]) PR_LX(u[6]) PR_LX(u[7]) }
+      if (MODE & 1) {
+        PR_DF(d[0]) PR_DF(d[1]) PR_DF(d[2]) PR_DF(d[3]) PR_DM(d[4]) PR_DF(d[5]) PR_DF(d[6]) PR_DF(d[7]) PR_DM(d[8]) PR_DA(d[9])
+        PR_DF(d[10]) PR_DF(d[11]) PR_DF(d[0]) PR_DF(d[1]) PR_DM(d[2]) PR_DF(d[3]) PR_DF(d[4]) PR_DF(d[5]) PR_DM(d[6]) PR_DA(d[7])
+        PR_DF(d[8]) PR_DF(d[9]) PR_DF(d[10]) PR_DF(d[11]) PR_DF(d[0]) PR_DF(d[1])
+      }
+    }
+    if (MODE & 32) { const double2 t = sh[(threadIdx.x + 3 * it) & 127]; ld += t.x; }
+  }
+  const long long t1 = clock64();
+  double acc = ld + cv[0] + cv[1] + cv[2] + rs;
+  uint32_t ua = 0;
+#pragma unroll
+  for (int j = 0; j < 12; ++j) acc += d[j];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) ua ^= u[j];
+  if (acc + static_cast<double>(ua) == 12345.0) out[threadIdx.x] = static_cast<float>(acc);
+  if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
+#define DEFINE_MIX_ROW(fn, kern)                                                                       \
+  template <int MODE>                                                                                  \
+  double fn(const Dev& d, int ctas_per_sm) {                                                           \
+    const int iters = 10000, grid = d.n_sm * ctas_per_sm;                                              \
+    kern<MODE><<<grid, 128>>>(200, d.in, d.out, d.cyc);                                                \
+    kern<MODE><<<grid, 128>>>(iters, d.in, d.out, d.cyc);                                              \
+    CK(cudaDeviceSynchronize());                                                                       \
+    std::vector<long long> c(grid);                                                                    \
+    CK(cudaMemcpy(c.data(), d.cyc, sizeof(long long) * grid, cudaMemcpyDeviceToHost));                 \
+    return static_cast<double>(*std::max_element(c.begin(), c.end())) / iters / ctas_per_sm;           \
+  }
+DEFINE_MIX_ROW(heun_mix, heun_mix_kernel)
+DEFINE_MIX_ROW(f64_mix, f64_mix_kernel)
+
+// ---------------------------------------------------------------------------------------------
+// Sixth table: dependent-issue latency.  ONE warp, one chain: every instruction waits for the one before.
+// Cycles per link of the chain (SM clocks), the quantity that bounds the small-ensemble kernel, where one
+// warp per scheduler integrates and nothing hides the recurrence v_n -> x_{n+1} -> force -> v_{n+2}.
+// ---------------------------------------------------------------------------------------------
+enum Chain { CH_FFMA, CH_FMUL, CH_FORCE, CH_COS, CH_DFMA, CH_IMADW, CH_LOP3, CH_LDS, CH_EMSTEP, N_CHAINS };
+static const char* CHAIN_NAME[N_CHAINS] = {
+    "FFMA -> FFMA", "FMUL -> FMUL", "FFMA -> FMUL.RZ -> MUFU.COS -> FFMA -> FFMA (force of x)",
+    "FMUL.RZ -> MUFU.COS", "DFMA -> DFMA", "IMAD.WIDE -> LOP3 (one Philox half round)", "LOP3 -> LOP3",
+    "LDS -> FFMA (shared-memory load to use)", "EM recurrence: v -> x -> force -> a_v -> v (two steps)"};
+
+template <int CH>
+__global__ void __launch_bounds__(32) chain_kernel(int iters, const float* __restrict__ in,
+                                                   float* __restrict__ out, long long* __restrict__ cycles) {
+  __shared__ float sh[64];
+  float x = in[4] + threadIdx.x * 1e-3f, v = in[5];
+  const float fb = in[0], fc = in[1];
+  double dx = x;
+  const double db = fb, dc = fc;
+  uint32_t u = __float_as_uint(in[2]) | 1u;
+  const uint32_t ub = __float_as_uint(in[3]);
+  sh[threadIdx.x] = fc;
+  sh[threadIdx.x + 32] = fc;
+  __syncthreads();
+  const long long t0 = clock64();
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+      if (CH == CH_FFMA) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(x) : "f"(fb), "f"(fc));
+      if (CH == CH_FMUL) asm volatile("mul.rn.f32 %0, %0, %1;" : "+f"(x) : "f"(fb));
+      if (CH == CH_FORCE)
+        asm volatile("{\n\t.reg .f32 a, c, p;\n\tfma.rn.f32 a, %0, %1, %2;\n\tcos.approx.ftz.f32 c, a;\n\t"
+                     "fma.rn.f32 p, c, %1, %2;\n\tfma.rn.f32 %0, p, c, %2;\n\t}" : "+f"(x) : "f"(fb), "f"(fc));
+      if (CH == CH_COS) asm volatile("cos.approx.ftz.f32 %0, %0;" : "+f"(x));
+      if (CH == CH_DFMA) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(dx) : "d"(db), "d"(dc));
+      if (CH == CH_IMADW)
+        asm volatile("{\n\t.reg .u64 p;\n\t.reg .u32 lo, hi;\n\tmul.wide.u32 p, %0, 0xD2511F53;\n\t"
+                     "mov.b64 {lo, hi}, p;\n\tlop3.b32 %0, lo, hi, %1, 0x96;\n\t}" : "+r"(u) : "r"(ub));
+      if (CH == CH_LOP3) asm volatile("lop3.b32 %0, %0, %1, %1, 0x96;" : "+r"(u) : "r"(ub));
+      if (CH == CH_LDS) {
+        float t;
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(t) : "r"(static_cast<uint32_t>(__cvta_generic_to_shared(sh)) +
+                                                                 ((__float_as_uint(x) & 31u) << 2)));
+        asm volatile("fma.rn.f32 %0, %1, %2, %0;" : "+f"(x) : "f"(t), "f"(fb));
+      }
+      if (CH == CH_EMSTEP) {
+        // two Euler-Maruyama steps of (x, v) with the force from the OLD position: x' = x + dt v,
+        // v' = v + dt (g v + k1 c + k2 c^2) + noise; e dropped (its chain is shorter)
+        asm volatile("{\n\t.reg .f32 a, c, p, f, w;\n\t"
+                     "fma.rn.f32 a, %0, %2, %3;\n\tcos.approx.ftz.f32 c, a;\n\tfma.rn.f32 p, c, %2, %3;\n\t"
+                     "fma.rn.f32 f, p, c, %3;\n\tfma.rn.f32 w, %2, %1, f;\n\tfma.rn.f32 %0, %3, %1, %0;\n\t"
+                     "fma.rn.f32 w, %3, w, %1;\n\tfma.rn.f32 %1, %2, %3, w;\n\t}"
+                     : "+f"(x), "+f"(v) : "f"(fb), "f"(fc));
+      }
+    }
+  }
+  const long long t1 = clock64();
+  if (static_cast<double>(x) + v + dx + u == 12345.0) out[threadIdx.x] = x;
+  if (threadIdx.x == 0) cycles[0] = t1 - t0;
+}
+
+template <int CH>
+void chain_row(const Dev& d) {
+  const int iters = 4000;
+  chain_kernel<CH><<<1, 32>>>(100, d.in, d.out, d.cyc);
+  chain_kernel<CH><<<1, 32>>>(iters, d.in, d.out, d.cyc);
+  CK(cudaDeviceSynchronize());
+  long long c = 0;
+  CK(cudaMemcpy(&c, d.cyc, sizeof(c), cudaMemcpyDeviceToHost));
+  std::printf("%-72s %8.2f\n", CHAIN_NAME[CH], static_cast<double>(c) / iters / 16);
+}
+
 int main() {
   Dev d;
   cudaDeviceProp p;
@@ -305,7 +549,7 @@ int main() {
   CK(cudaMalloc(&d.out, 4096));
   CK(cudaMalloc(&d.cyc, sizeof(long long) * d.n_sm * 16));
   std::printf("# warp-lane operations per clock per SM (slowest CTA), 8 independent chains/thread\n");
-  std::printf("%-22s %8s %8s %8s\n", "instruction", "8 warps", "16 warps", "32 warps");
+  std::printf("%-22s %8s %8s %8s %8s\n", "instruction", "4 warps", "8 warps", "16 warps", "32 warps");
   single<FFMA_RRR>(d); single<FFMA_RRC>(d); single<FFMA_RIR>(d); single<FMUL_RR>(d);
   single<FADD_RR>(d); single<IMAD_LO>(d); single<IMAD_WIDE_R>(d); single<IMAD_WIDE_I>(d);
   single<LOP3_XOR3>(d); single<IADD3>(d); single<SHF_R>(d);
@@ -336,6 +580,12 @@ int main() {
   mix<I2F_, MUFU_LG2>(d);
   mix<I2F_, LOP3_XOR3>(d);
   mix<I2F_, FFMA_RRR>(d);
+  std::printf("# the same one-to-one mixes with ONE warp per scheduler (4 warps/SM): what a single warp can issue\n");
+  mix1<FFMA_RRR, LOP3_XOR3>(d);
+  mix1<FFMA_RRR, FMUL_RR>(d);
+  mix1<FFMA_RRR, MUFU_COS>(d);
+  mix1<FFMA2_, FFMA_RRR>(d);
+  mix1<FFMA2_, LOP3_XOR3>(d);
   std::printf("# the fp32 Euler-Maruyama step-loop mix as independent chains: SM cycles per warp and scheduler for\n"
               "# one Philox block (four steps); the step kernel itself: kernel time x clock / (steps / 4) / warps per scheduler\n");
   std::printf("%-44s %8s %8s %8s\n", "instructions per block", "4 CTA/SM", "9 CTA/SM", "12 CTA/SM");
@@ -348,5 +598,35 @@ int main() {
   loop_mix_row<6>(d, "Philox + MUFU");
   loop_mix_row<7>(d, "FP32 + Philox + MUFU");
   loop_mix_row<15>(d, "all (the step loop's mix, 118 instructions)");
+  std::printf("# the fp32 Heun + tilt step-loop mix (config[3]) as independent chains: SM cycles per warp and scheduler\n"
+              "# for one Philox block (four steps)\n");
+  std::printf("%-44s %8s %8s %8s\n", "instructions per block", "4 CTA/SM", "8 CTA/SM", "12 CTA/SM");
+#define ROW(fn, mode, name) std::printf("%-44s %8.1f %8.1f %8.1f\n", name, fn<mode>(d, 4), fn<mode>(d, 8), fn<mode>(d, 12));
+  ROW(heun_mix, 1, "120 FFMA/FADD/FMUL")
+  ROW(heun_mix, 2, "16 (IMAD.WIDE + LOP3)")
+  ROW(heun_mix, 4, "10 (FMUL.RZ + MUFU.COS) + 6 MUFU")
+  ROW(heun_mix, 3, "FP32 + Philox")
+  ROW(heun_mix, 7, "FP32 + Philox + MUFU")
+  ROW(heun_mix, 15, "FP32 + Philox + MUFU + 14 ALU")
+  ROW(heun_mix, 31, "all (+ 4 LDG, LDS.128, F2I, I2F: 199 instr.)")
+#undef ROW
+  std::printf("# the fp64 Euler-Maruyama step-loop mix (config[4]) as independent chains: SM cycles per warp and scheduler\n"
+              "# for one Philox block (four steps)\n");
+  std::printf("%-44s %8s %8s %8s\n", "instructions per block", "3 CTA/SM", "5 CTA/SM", "8 CTA/SM");
+#define ROW(fn, mode, name) std::printf("%-44s %8.1f %8.1f %8.1f\n", name, fn<mode>(d, 3), fn<mode>(d, 5), fn<mode>(d, 8));
+  ROW(f64_mix, 1, "114 DFMA + 22 DMUL + 12 DADD")
+  ROW(f64_mix, 2, "16 (IMAD.WIDE + LOP3)")
+  ROW(f64_mix, 3, "FP64 + Philox")
+  ROW(f64_mix, 17, "FP64 + 20 IMAD (moves on the FMA pipe)")
+  ROW(f64_mix, 9, "FP64 + 40 ALU")
+  ROW(f64_mix, 5, "FP64 + 6 I2F.F64 + 2 MUFU.RSQ64H")
+  ROW(f64_mix, 33, "FP64 + 5 LDS.128")
+  ROW(f64_mix, 19, "FP64 + Philox + 20 IMAD")
+  ROW(f64_mix, 63, "all (the fp64 loop's mix, 257 instructions)")
+  ROW(f64_mix, 47, "all but the 20 IMAD")
+#undef ROW
+  std::printf("# dependent-issue latency: one warp, one chain; SM cycles per link\n");
+  chain_row<CH_FFMA>(d); chain_row<CH_FMUL>(d); chain_row<CH_COS>(d); chain_row<CH_FORCE>(d);
+  chain_row<CH_EMSTEP>(d); chain_row<CH_DFMA>(d); chain_row<CH_IMADW>(d); chain_row<CH_LOP3>(d); chain_row<CH_LDS>(d);
   return 0;
 }
