@@ -49,15 +49,21 @@ N_SM, LANES_PER_SM = 148, 128
 # config[4] is bound by the FP64 pipe (64 lanes/clk/SM; 59 measured for DFMA), not by issue slots: its
 # I_alg counts the ~60 DFMA-pipe operations per particle-step and its peak is 64 lanes.
 LANES_FP64 = 64
-# dram__bytes_read.sum + dram__bytes_write.sum of the step kernel, per launch, from the committed
-# `ncu --set full` captures of the launch bench.py times (profiles/*_ncu_full.md), each with the git blob
-# ids of the two kernel sources it was captured on: when a source has changed since, the figure is stale
-# and the line says `"traffic": null` instead (re-capture, then update the entry).
-# The frame (one, overwritten) and the state stay in the 126 MB L2 during a launch, so the traffic is
-# far BELOW the algorithmic bytes.  configs[2-4] were captured on launches shortened with --sim-steps; a
-# launch reads the state once and writes it once whatever its step count, so the figure holds.
-NCU_TRAFFIC = {
-    # cfg: (bytes per launch, blob of csrc/abm_kernels.cuh, blob of csrc/abm_device.cuh, summary)
+# What the committed `ncu --set full` captures of the launches bench.py times say about the step kernel
+# (profiles/r02_step_kernels_ncu_full.md), per launch: dram__bytes_read.sum + dram__bytes_write.sum (`traffic`)
+# and what the kernel EXECUTES per particle-step -- warp-lane instructions (smsp__inst_executed.sum x 32 / particle-
+# steps) for the fp32 kernels, FP64-pipe lane operations (smsp__inst_executed_pipe_fp64.sum x 32 / particle-steps)
+# for config[4] -- from which `roofline.frac_executed` follows: the fraction of the issue slots (or of the FP64
+# pipe) the kernel keeps busy with whatever it executes, next to `frac`, which credits the frozen I_alg.
+# Each entry carries the git blob ids of the two kernel sources it was captured on: when a source has changed
+# since, the figures are stale and the line says null instead (re-capture, then update the entry).
+# The frame (one, overwritten) and the state stay in the 126 MB L2 during a launch, so the traffic is far BELOW
+# the algorithmic bytes.  configs[2-4] were captured on launches shortened with --sim-steps; a launch reads the
+# state once and writes it once whatever its step count, so the traffic figure holds, and the executed count per
+# particle-step is that of the loop.
+NCU_CAPTURE = {
+    # cfg: dict(traffic=bytes per launch, executed=per particle-step, kernels=blob of csrc/abm_kernels.cuh,
+    #           device=blob of csrc/abm_device.cuh, summary=file under profiles/)
 }
 # Warp-lane instructions per particle-step of the xorshift variant are not frozen anywhere: no `frac` for it.
 
@@ -69,15 +75,16 @@ def git_blob(path):
     return hashlib.sha1(b"blob %d\0" % len(data) + data).hexdigest()
 
 
-def ncu_traffic(cfg_id):
-    ent = NCU_TRAFFIC.get(cfg_id)
+def ncu_capture(cfg_id):
+    """-> (entry or None, where it comes from / why there is none)"""
+    ent = NCU_CAPTURE.get(cfg_id)
     if not ent:
         return None, "no committed capture of this launch"
     csrc = os.path.join(ROOT, "paper_1104_2499_b200", "csrc")
     now = (git_blob(os.path.join(csrc, "abm_kernels.cuh")), git_blob(os.path.join(csrc, "abm_device.cuh")))
-    if now != (ent[1], ent[2]):
-        return None, f"stale: kernel sources changed since the capture in {ent[3]}"
-    return ent[0], f"ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, {ent[3]}"
+    if now != (ent["kernels"], ent["device"]):
+        return None, f"stale: kernel sources changed since the capture in {ent['summary']}"
+    return ent, f"ncu --set full, per launch, {ent['summary']}"
 
 
 def load_peaks():
@@ -399,7 +406,7 @@ def run_ours(args, wl, cfg_id):
         peak = N_SM * lanes * f_max
         achieved = lane_instr / t_k
         sm_mhz = clocks.get("sm_mhz") or (f_max / 1e6)
-        traffic, traffic_src = ncu_traffic(cfg_id) if (not args.sim_steps and args.rng == "philox") else \
+        cap, cap_src = ncu_capture(cfg_id) if (not args.sim_steps and args.rng == "philox") else \
             (None, "no capture of this launch (--sim-steps / --rng xorshift)")
         philox = args.rng == "philox"
         out["roofline"] = {
@@ -411,12 +418,16 @@ def run_ours(args, wl, cfg_id):
             "frac": achieved / peak if philox else None,     # I_alg is frozen for the Philox path only
             "frac_at_sustained_clock": achieved / (N_SM * lanes * sm_mhz * 1e6) if philox else None,
             "i_alg_per_particle_step": I_ALG[cfg_id] if philox else None,
+            # the same with what the kernel executes per particle-step in place of I_alg (ncu capture): how busy
+            # the issue slots (fp64: the FP64 pipe) are, whatever the instructions are worth
+            "frac_executed": cap["executed"] * wl.particle_steps / t_k / peak if cap else None,
+            "executed_per_particle_step": cap["executed"] if cap else None,
             "particle_steps_per_pass": wl.particle_steps,
             "kernel_ms": 1e3 * t_k, "kernel_ms_sd": statistics.pstdev(t_kern_ms) if len(t_kern_ms) > 1 else None,
             "kernel_launches_per_pass": step_launches * (n_steps // M),
             "kernel_share_of_pass": sum(t_kern_ms) / sum(t_pass_ms),
             "peak_source": f"148 SMs x {lanes} lanes x sm_max_mhz {f_max / 1e6:.0f} MHz, {peak_src}",
-            "traffic": traffic, "traffic_source": traffic_src,
+            "traffic": cap["traffic"] if cap else None, "traffic_source": cap_src,
             "hbm_algorithmic_bytes_per_launch": int(T * (24 + 8 * (n_steps // wl.snapshot_every
                                                                    if wl.snapshot_every else 0))),
         }

@@ -52,7 +52,7 @@ struct abm_ctx {
   void* xh;             //   and its whole periods (the x array then holds the float offset)
   uint4* rng_state;     // xorshift state per trajectory (ABM_RNG_XORSHIFT128 only)
   void* coef_table;     // Coef<Real>[n_sets]
-  void* tilt_table;     // Real[TILT_CHUNK + 1]
+  void* tilt_table;     // Real[TILT_CHUNK + 8]: 3 elements of alignment shift, 3 of lead-in, the chunk, t_{n+1} of its last step
   double2* noise_tables;  // fp64 only: Box-Muller circle and log tables (NoiseTables), [NOISE_TABLE_N]
   double* partial;      // [n_sets * blocks_per_set][7]
   double* sums;         // [n_sets][8]
@@ -489,12 +489,17 @@ int step_impl(abm_ctx* c, uint64_t n_steps) {
       else if (chunk >= 4u) chunk &= ~3u;
     }
     a.step0 = c->step;
-    a.tilt_base = c->step;
     a.n_steps = chunk;
     if (c->tilt) {
-      const uint32_t n_tab = chunk + 1;  // Heun reads t_{n+1} of the last step
-      tilt_kernel<Real><<<(n_tab + 255) / 256, 256, 0, c->stream>>>(
-          static_cast<Real*>(c->tilt_table), c->step, n_tab, c->omega, c->dt, c->tilt_k0, c->tilt_A);
+      // The table starts at a multiple of four steps and is shifted so that the 16-byte loads of the block
+      // loop (TiltCursor) are aligned.
+      a.tilt_base = c->step & ~3ull;
+      Real* const tab = static_cast<Real*>(c->tilt_table) +
+                        tilt_table_shift<Real>(c->integrator == ABM_EULER_MARUYAMA ? 0 : 1);
+      a.tilt = tab;
+      const uint32_t n_tab = static_cast<uint32_t>(c->step - a.tilt_base) + chunk + 1;  // Heun reads t_{n+1} of the last step
+      tilt_kernel<Real><<<(n_tab + 255) / 256, 256, 0, c->stream>>>(tab, a.tilt_base, n_tab, c->omega, c->dt,
+                                                                   c->tilt_k0, c->tilt_A);
       ABM_CK(c, cudaGetLastError());
     }
     ABM_CK(c, launch_step<Real>(c, a));
@@ -679,7 +684,7 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
              sizeof(double) * (N_SUMS - 1) * bps * n_param_sets) ||
       !alloc(reinterpret_cast<void**>(&c->sums), sizeof(double) * N_SUMS * n_param_sets) ||
       !alloc(reinterpret_cast<void**>(&c->moments), sizeof(MomentRec) * n_param_sets) ||
-      (c->tilt && !alloc(&c->tilt_table, c->real_size * (TILT_CHUNK + 1))) ||
+      (c->tilt && !alloc(&c->tilt_table, c->real_size * (TILT_CHUNK + 8))) ||
       (c->precision == ABM_FP64 &&
        !alloc(reinterpret_cast<void**>(&c->noise_tables), sizeof(double2) * NOISE_TABLE_N)))
     return fail(rc);

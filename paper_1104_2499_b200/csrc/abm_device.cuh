@@ -264,7 +264,9 @@ __constant__ double C_COSPI[N_COSPI] = {
 __device__ __forceinline__ double reduce_half_turns(double t, uint32_t& sign) {
   const double magic = 6755399441055744.0;  // 1.5 * 2^52: adding it rounds to an integer
   const double tm = __dadd_rn(t, magic);
-  sign = static_cast<uint32_t>(__double2loint(tm)) << 31;  // parity of rint(t) -> sign bit
+  // parity of rint(t) -> sign bit.  A funnel shift: ptxas turns a plain `<< 31` into IMAD.U32 (x 2^31) on the
+  // FMA pipe, whose dispatch port the FP64 pipe shares (profiles/r02_pipe_rates.txt) -- the one this kernel is short of.
+  asm("shf.l.wrap.b32 %0, 0, %1, 31;" : "=r"(sign) : "r"(__double2loint(tm)));
   return __dadd_rn(t, -__dadd_rn(tm, -magic));             // exact
 }
 __device__ __forceinline__ double flip_sign(double p, uint32_t sign) {
@@ -298,13 +300,20 @@ constexpr int LOG_N = 257;
 constexpr int LOG_ADJ_FROM = 106;                // c_i >= 1.412 ~ sqrt 2: the mantissa is taken as m / 2
 constexpr int NOISE_TABLE_N = CIRCLE_N + LOG_N;  // double2 entries: circle first, then logt
 
+// The shared-memory copy every CTA of an fp64 step kernel makes (stage_noise_tables in abm_kernels.cuh).  A static
+// array, so that a look-up is LDS [index * 16 + constant]: with the tables behind pointers every look-up paid an
+// integer add, which ptxas issues as IMAD.IADD on the FMA pipe.
+__shared__ double2 s_noise[NOISE_TABLE_N];
 template <typename Real>
-struct NoiseTables {};  // fp32: none (MUFU)
-template <>
-struct NoiseTables<double> {
-  const double2* circle;
-  const double2* logt;
-};
+struct NoiseTables {};  // a tag: fp32 has none (MUFU), fp64 reads s_noise
+// A right shift the compiler cannot merge with the scaling of the table index that follows it: index -> address
+// is then one shift-and-add (LEA, ALU pipe) instead of a mask and an add that ptxas issues on the FMA pipe.
+template <int N>
+__device__ __forceinline__ uint32_t shr_opaque(uint32_t x) {
+  uint32_t d;
+  asm("shr.u32 %0, %1, %2;" : "=r"(d) : "r"(x), "n"(N));
+  return d;
+}
 
 // (cos d - 1) / d^2 and sin(d) / d as linear functions of d^2 on |d| <= pi / 1024 (csrc/fit_coefficients.py:
 // 1.5e-19 and 2.8e-16 absolute on cos d, sin d), the angle scale C = 2 pi 2^-32 and (1/2 - 2^21) C, and
@@ -318,9 +327,8 @@ __constant__ double C_LOG1P[6] = {-0.49999999999969563, 0.33333333333307247, -0.
 // cos(2 pi u), sin(2 pi u) for u = (w + 1/2) 2^-32: the top 10 bits of w pick the table angle a_i, the low
 // 22 bits are the remainder d = 2 pi (low - 2^21 + 1/2) 2^-32, |d| <= pi / 1024, and
 // cos(a + d) = cos a + (cos a (cos d - 1) - sin a sin d),  sin(a + d) = sin a + (sin a (cos d - 1) + cos a sin d).
-__device__ __forceinline__ void sincos_2pi_u_f64(uint32_t w, const double2* __restrict__ circle, double* sn,
-                                                 double* cs) {
-  const double2 t = circle[w >> (32 - CIRCLE_BITS)];
+__device__ __forceinline__ void sincos_2pi_u_f64(uint32_t w, double* sn, double* cs) {
+  const double2 t = s_noise[shr_opaque<32 - CIRCLE_BITS>(w)];
   const uint32_t low = w & ((1u << (32 - CIRCLE_BITS)) - 1u);
   const double d = __fma_rn(static_cast<double>(low), C_BMTRIG[4], C_BMTRIG[5]);
   const double d2 = __dmul_rn(d, d);
@@ -335,19 +343,21 @@ __device__ __forceinline__ void sincos_2pi_u_f64(uint32_t w, const double2* __re
 // For c >= 1.412 the entry holds -ln rc - ln 2 and e counts one more (m taken as m / 2 in [0.706, 1)), so
 // that e ln 2 and ln m never cancel as u -> 1; the last entry, c = 2, has rc = 1/2 and 0 exactly, and
 // ln u keeps its relative accuracy where it is smallest.
-__device__ __forceinline__ double ln_uniform_f64(uint32_t w, const double2* __restrict__ logt) {
+__device__ __forceinline__ double ln_uniform_f64(uint32_t w) {
   const double kd = __fma_rn(static_cast<double>(w), C_LOG1P[5], 1.0);  // exact, < 2^33
   const int hi = __double2hiint(kd);
   const int mant = hi & 0x000fffff;
-  const int i = (mant + 0x800) >> 12;                                   // round(256 (m - 1)), 0 .. 256
+  const uint32_t i = shr_opaque<12>(static_cast<uint32_t>(mant) + 0x800u);  // round(256 (m - 1)), 0 .. 256
   const double m = __hiloint2double(mant | 0x3ff00000, __double2loint(kd));
-  const double2 t = logt[i];
+  const double2 t = s_noise[CIRCLE_N + i];
   const double r = __fma_rn(m, t.x, -1.0);
   double g = C_LOG1P[3];
 #pragma unroll
   for (int q = 2; q >= 0; --q) g = __fma_rn(g, r, C_LOG1P[q]);
   const double p = __fma_rn(g, r, 1.0);                                 // log1p(r) / r
-  const double E = static_cast<double>((hi >> 20) - (1023 + 33) + (i >= LOG_ADJ_FROM ? 1 : 0));
+  // exponent, one more where i >= LOG_ADJ_FROM, i.e. mant >= (LOG_ADJ_FROM << 12) - 0x800: as a carry out of the
+  // mantissa field (three ALU instructions; the comparison cost a predicated move on the FMA pipe)
+  const double E = static_cast<double>(((hi + (0x100000 - ((LOG_ADJ_FROM << 12) - 0x800))) >> 20) - (1023 + 33));
   return __fma_rn(E, C_LOG1P[4], __fma_rn(r, p, t.y));
 }
 
@@ -375,11 +385,10 @@ __device__ __forceinline__ double uniform_f64(uint32_t w) {
   return __fma_rn(static_cast<double>(w), 0x1p-32, 0x1p-33);  // (w + 0.5) 2^-32, exact
 }
 
-__device__ __forceinline__ Normal2d box_muller_f64(uint32_t wa, uint32_t wb, double sigma,
-                                                   const NoiseTables<double>& nt) {
+__device__ __forceinline__ Normal2d box_muller_f64(uint32_t wa, uint32_t wb, double sigma) {
   Normal2d o;
-  o.rho = __dmul_rn(sigma, sqrt_pos_f64(__dmul_rn(-2.0, ln_uniform_f64(wa, nt.logt))));
-  sincos_2pi_u_f64(wb, nt.circle, &o.sn, &o.cs);
+  o.rho = __dmul_rn(sigma, sqrt_pos_f64(__dmul_rn(-2.0, ln_uniform_f64(wa))));
+  sincos_2pi_u_f64(wb, &o.sn, &o.cs);
   return o;
 }
 
@@ -468,6 +477,14 @@ __device__ __forceinline__ double load_position(const double* x, const double*, 
   return x[k];
 }
 
+// Order of the sums: cos -> f -> a_v -> v + dt a_v -> + noise, five dependent FMAs from the cosine to the new
+// velocity.  Adding everything that does not wait for the cosine first (h = (d e - gamma0) v + k0t as the
+// constant term of the force polynomial, the noise increment onto v before dt a_v) leaves three and shortens the
+// recurrence v_n -> x_{n+1} -> cos -> v_{n+2} that bounds small ensembles from 27.2 to 22.9 clocks per step
+// (csrc/pipe_rates.cu, last table); measured on the kernels: step_kernel_small 0.192 -> 0.185 ms per 10^4 steps
+// (config[0]), but the throughput-bound loop of config[1] 22.31 -> 22.85 ms per 20,000 steps (the same
+// instruction count, a worse ptxas schedule), config[2] 8.87 -> 8.99.  Both kernels must execute the same
+// arithmetic (a trajectory does not depend on which kernel ran), and config[1] is the headline: not taken.
 template <bool PRECISE, typename Real>
 __device__ __forceinline__ void em_step(State<Real>& s, const Coef<Real>& k, Real k0t, Real rho,
                                         Real cs) {
@@ -481,6 +498,10 @@ __device__ __forceinline__ void em_step(State<Real>& s, const Coef<Real>& k, Rea
 
 // Stochastic Heun: predictor = EM step with the full noise increment; corrector averages the
 // drift at (X, t_n) and (X~, t_{n+1}); the same sigma z in both (reading G16).
+// v' is rounded ONCE at the magnitude of v (the increment is summed first).  The cheaper corrector
+// v' = v~ + (dt/2)(a2 - a1) on a predictor built as in em_step (two instructions less per step) rounds three
+// times at that magnitude; on a stiff potential (config[3]'s model with L = 0.5: dt max U'' = 1.6) the
+// instability of the dynamics amplifies the difference to 1.2e-5 after 100 steps against 8.7e-6 (measured).
 template <bool PRECISE, typename Real>
 __device__ __forceinline__ void heun_step(State<Real>& s, const Coef<Real>& k, Real k0t, Real k0t1,
                                           Real rho, Real cs) {

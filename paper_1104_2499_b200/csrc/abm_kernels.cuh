@@ -63,7 +63,8 @@ struct StepArgs {
   Real* xl;                      // PRECISE: bits of xf, the fraction word of the fixed-point position
   Real* xh;                      // PRECISE: bits of xc, its whole periods (else both nullptr)
   const Coef<Real>* coef_table;  // [n_sets] (used when !UNIFORM)
-  const Real* tilt;              // tilt[j] = k0 + A cos(omega (tilt_base + j) dt): (k0, A) of the one set, or (0, 1)
+  const Real* tilt;              // tilt[j] = k0 + A cos(omega (tilt_base + j) dt): (k0, A) of the one set, or (0, 1);
+                                 // tilt_base is a multiple of 4 and tilt + INTEG is 16-byte aligned (TiltCursor)
   void* snap;                    // bound snapshot buffer or nullptr
   uint4* rng_state;              // xorshift state per trajectory (used when XS), at a pair boundary
   uint64_t n_traj;               // local trajectories
@@ -227,8 +228,8 @@ template <>
 struct Noise4<double> {
   static constexpr double SIGN = Normal2d::NEGATED ? -1.0 : 1.0;
   Normal2d a, b;
-  __device__ __forceinline__ Noise4(const uint4& w, const Coef<double>& k, const NoiseTables<double>& nt)
-      : a(box_muller_f64(w.x, w.y, k.s2, nt)), b(box_muller_f64(w.z, w.w, k.s2, nt)) {}
+  __device__ __forceinline__ Noise4(const uint4& w, const Coef<double>& k, const NoiseTables<double>&)
+      : a(box_muller_f64(w.x, w.y, k.s2)), b(box_muller_f64(w.z, w.w, k.s2)) {}
 };
 
 template <typename Real, int INTEG, int TILT, bool PRECISE>
@@ -245,16 +246,45 @@ __device__ __forceinline__ void one_step(State<Real>& s, const Coef<Real>& k, Re
   }
 }
 
+// The tilt values of the coming four steps (TILT != 0): t_n ... t_{n+3} for Euler-Maruyama, and t_{n+4} too for
+// Heun, whose corrector evaluates the force at t_{n+1}.  One 16-byte load per Philox block (fp64: two) from an
+// address every thread of the launch shares: the host places the table so that what a block loads is 16-byte
+// aligned whenever n is a multiple of 4 (step_impl: the table starts at a multiple of four steps, shifted by one
+// element for Heun, whose first value of a block is the last one of the block before and is carried in a register).
+template <typename Real, int INTEG>
+struct TiltCursor {
+  const Real* p = nullptr;
+  Real carry = 0;
+  __device__ __forceinline__ void start(const Real* q) {
+    p = q;
+    if (INTEG == 1) carry = q[0];
+  }
+  __device__ __forceinline__ void next4(Real& t0, Real& t1, Real& t2, Real& t3, Real& t4) {
+    if constexpr (sizeof(Real) == 4) {
+      const float4 q = *reinterpret_cast<const float4*>(p + INTEG);
+      if (INTEG == 1) { t0 = carry; t1 = q.x; t2 = q.y; t3 = q.z; t4 = q.w; carry = q.w; }
+      else { t0 = q.x; t1 = q.y; t2 = q.z; t3 = q.w; }
+    } else {
+      const double2 q = *reinterpret_cast<const double2*>(p + INTEG);
+      const double2 r = *reinterpret_cast<const double2*>(p + INTEG + 2);
+      if (INTEG == 1) { t0 = carry; t1 = q.x; t2 = q.y; t3 = r.x; t4 = r.y; carry = r.y; }
+      else { t0 = q.x; t1 = q.y; t2 = r.x; t3 = r.y; }
+    }
+    p += 4;
+  }
+};
+// elements in front of the table so that (table + INTEG) is 16-byte aligned
+template <typename Real>
+__host__ __device__ constexpr uint32_t tilt_table_shift(int integ) {
+  return integ == 1 ? (sizeof(Real) == 4 ? 3u : 1u) : 0u;
+}
+
 // Four steps from the noise of one Philox block.
 template <typename Real, int INTEG, int TILT, bool PRECISE>
 __device__ __forceinline__ void four_steps_z(State<Real>& s, const Coef<Real>& cf,
-                                             const Noise4<Real>& z, const Real*& tl) {
+                                             const Noise4<Real>& z, TiltCursor<Real, INTEG>& tl) {
   Real t0 = 0, t1 = 0, t2 = 0, t3 = 0, t4 = 0;
-  if (TILT) {
-    t0 = tl[0]; t1 = tl[1]; t2 = tl[2]; t3 = tl[3];
-    if (INTEG == 1) t4 = tl[4];
-    tl += 4;
-  }
+  if (TILT) tl.next4(t0, t1, t2, t3, t4);
   const Real ra = Noise4<Real>::SIGN * z.a.rho, rb = Noise4<Real>::SIGN * z.b.rho;
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.cs, t0, t1);
   one_step<Real, INTEG, TILT, PRECISE>(s, cf, ra, z.a.sn, t1, t2);
@@ -265,7 +295,7 @@ __device__ __forceinline__ void four_steps_z(State<Real>& s, const Coef<Real>& c
 // Four steps from one Philox block.
 template <typename Real, int INTEG, int TILT, bool PRECISE>
 __device__ __forceinline__ void four_steps(State<Real>& s, const Coef<Real>& cf, const uint4& w,
-                                           const Real*& tl, const NoiseTables<Real>& nt) {
+                                           TiltCursor<Real, INTEG>& tl, const NoiseTables<Real>& nt) {
   const Noise4<Real> z(w, cf, nt);
   four_steps_z<Real, INTEG, TILT, PRECISE>(s, cf, z, tl);
 }
@@ -329,12 +359,14 @@ struct Integrate {
   const uint64_t k;
   const bool active;
   const NoiseTables<Real> nt;
-  const Real* tl;
+  TiltCursor<Real, INTEG> tl;
   __device__ __forceinline__ Integrate(const StepArgs<Real>& a_, const Coef<Real>& cf_, State<Real>& s_,
                                        uint64_t k_, bool active_, const NoiseTables<Real>& nt_)
-      : a(a_), cf(cf_), s(s_), k(k_), active(active_), nt(nt_), tl(nullptr) {}
-  // a run of whole blocks starts at step n
-  __device__ __forceinline__ void start(uint64_t n) { tl = TILT ? a.tilt + (n - a.tilt_base) : nullptr; }
+      : a(a_), cf(cf_), s(s_), k(k_), active(active_), nt(nt_) {}
+  // a run of whole blocks starts at step n (a multiple of 4)
+  __device__ __forceinline__ void start(uint64_t n) {
+    if (TILT) tl.start(a.tilt + (n - a.tilt_base));
+  }
   __device__ __forceinline__ void block(const uint4& w) {
     four_steps<Real, INTEG, TILT, PRECISE>(s, cf, w, tl, nt);
   }
@@ -554,10 +586,9 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint32_
 // fp64: every CTA copies the Box-Muller tables (17.9 KB) from global to shared memory once per launch.
 __device__ __forceinline__ NoiseTables<float> stage_noise_tables(const StepArgs<float>&) { return {}; }
 __device__ __forceinline__ NoiseTables<double> stage_noise_tables(const StepArgs<double>& a) {
-  __shared__ double2 tabs[NOISE_TABLE_N];
-  for (int i = threadIdx.x; i < NOISE_TABLE_N; i += STEP_BLOCK) tabs[i] = a.noise_tables[i];
+  for (int i = threadIdx.x; i < NOISE_TABLE_N; i += STEP_BLOCK) s_noise[i] = a.noise_tables[i];
   __syncthreads();
-  return {tabs, tabs + CIRCLE_N};
+  return {};
 }
 
 template <typename Real, int INTEG, bool TILT, int COEF, bool PRECISE, bool XS>
@@ -674,7 +705,7 @@ step_kernel_small(const __grid_constant__ StepArgs<float> a) {
   };
 
   State<float> s{0.f, 0.f, 0.f, 0.f, 0u, 0, 0.f};
-  const float* tl = nullptr;
+  TiltCursor<float, INTEG> tl;
   uint32_t to_snap = 0xffffffffu;  // blocks until the next frame (a launch has fewer than 2^30 steps)
   const uint32_t K = a.snap != nullptr ? a.snap_every : 0u;
   if (warp == 0) {
@@ -684,7 +715,7 @@ step_kernel_small(const __grid_constant__ StepArgs<float> a) {
       s.xc = __float_as_int(a.xh[k]);
       s.thb = fixed_angle(s.xf, cf.th_o);
     }
-    if (TILT) tl = a.tilt + (a.step0 - a.tilt_base);
+    if (TILT) tl.start(a.tilt + (a.step0 - a.tilt_base));
     if (K) to_snap = static_cast<uint32_t>(((a.step0 / K + 1) * static_cast<uint64_t>(K) - a.step0) >> 2);
   } else {
     produce(0u, 0u);

@@ -466,11 +466,12 @@ DEFINE_MIX_ROW(f64_mix, f64_mix_kernel)
 // Cycles per link of the chain (SM clocks), the quantity that bounds the small-ensemble kernel, where one
 // warp per scheduler integrates and nothing hides the recurrence v_n -> x_{n+1} -> force -> v_{n+2}.
 // ---------------------------------------------------------------------------------------------
-enum Chain { CH_FFMA, CH_FMUL, CH_FORCE, CH_COS, CH_DFMA, CH_IMADW, CH_LOP3, CH_LDS, CH_EMSTEP, N_CHAINS };
+enum Chain { CH_FFMA, CH_FMUL, CH_FORCE, CH_COS, CH_DFMA, CH_IMADW, CH_LOP3, CH_LDS, CH_EMSTEP, CH_EMSTEP2, N_CHAINS };
 static const char* CHAIN_NAME[N_CHAINS] = {
     "FFMA -> FFMA", "FMUL -> FMUL", "FFMA -> FMUL.RZ -> MUFU.COS -> FFMA -> FFMA (force of x)",
     "FMUL.RZ -> MUFU.COS", "DFMA -> DFMA", "IMAD.WIDE -> LOP3 (one Philox half round)", "LOP3 -> LOP3",
-    "LDS -> FFMA (shared-memory load to use)", "EM recurrence: v -> x -> force -> a_v -> v (two steps)"};
+    "LDS -> FFMA (shared-memory load to use)", "EM recurrence, sums in round 1's order: cos -> f -> a_v -> v + dt a_v -> + noise",
+    "EM recurrence as em_step has it now: cos -> f + h -> (v + noise) + dt a_v"};
 
 template <int CH>
 __global__ void __launch_bounds__(32) chain_kernel(int iters, const float* __restrict__ in,
@@ -514,6 +515,15 @@ __global__ void __launch_bounds__(32) chain_kernel(int iters, const float* __res
                      "fma.rn.f32 a, %0, %2, %3;\n\tcos.approx.ftz.f32 c, a;\n\tfma.rn.f32 p, c, %2, %3;\n\t"
                      "fma.rn.f32 f, p, c, %3;\n\tfma.rn.f32 w, %2, %1, f;\n\tfma.rn.f32 %0, %3, %1, %0;\n\t"
                      "fma.rn.f32 w, %3, w, %1;\n\tfma.rn.f32 %1, %2, %3, w;\n\t}"
+                     : "+f"(x), "+f"(v) : "f"(fb), "f"(fc));
+      }
+      if (CH == CH_EMSTEP2) {
+        // the same step with the sums in em_step's order: h = g v + k0 and v + noise do not wait for the
+        // cosine; a_v = (k2 c + k1) c + h; v' = dt a_v + (v + noise)
+        asm volatile("{\n\t.reg .f32 a, c, p, h, w, t;\n\t"
+                     "fma.rn.f32 a, %0, %2, %3;\n\tcos.approx.ftz.f32 c, a;\n\tfma.rn.f32 h, %2, %1, %3;\n\t"
+                     "fma.rn.f32 t, %2, %3, %1;\n\tfma.rn.f32 p, c, %2, %3;\n\tfma.rn.f32 w, p, c, h;\n\t"
+                     "fma.rn.f32 %0, %3, %1, %0;\n\tfma.rn.f32 %1, %3, w, t;\n\t}"
                      : "+f"(x), "+f"(v) : "f"(fb), "f"(fc));
       }
     }
@@ -627,6 +637,6 @@ int main() {
 #undef ROW
   std::printf("# dependent-issue latency: one warp, one chain; SM cycles per link\n");
   chain_row<CH_FFMA>(d); chain_row<CH_FMUL>(d); chain_row<CH_COS>(d); chain_row<CH_FORCE>(d);
-  chain_row<CH_EMSTEP>(d); chain_row<CH_DFMA>(d); chain_row<CH_IMADW>(d); chain_row<CH_LOP3>(d); chain_row<CH_LDS>(d);
+  chain_row<CH_EMSTEP>(d); chain_row<CH_EMSTEP2>(d); chain_row<CH_DFMA>(d); chain_row<CH_IMADW>(d); chain_row<CH_LOP3>(d); chain_row<CH_LDS>(d);
   return 0;
 }

@@ -484,23 +484,35 @@ def test_moment_reduction_matches_numpy(abm, oracle, n_particles, n_sets):
     assert np.array_equal(back.view(np.uint8), m.view(np.uint8))
 
 
-def _moment_check(name, got, sub, x0):
-    """got: abm_moment record of the GPU ensemble; sub: oracle state [N_sub, 3] of a subset."""
+def _moment_check(name, got, sub, x0, n_gpu=None):
+    """got: abm_moment record of the GPU ensemble; sub: oracle state [N_orc, 3] of an oracle sample of the same
+    model.  The bar is BASELINE.json's: 3 standard errors + 1e-4 relative.  n_gpu = None: the oracle sample is the
+    smaller one (a subset of the GPU's trajectories) and the standard error is the subset's.  n_gpu = N: the oracle
+    sample is much larger than the GPU ensemble of N trajectories and independent of it (other trajectory indices),
+    and the standard error is that of an N-trajectory ensemble, with the spread taken from the oracle sample."""
     x, v, e = sub[:, 0], sub[:, 1], sub[:, 2]
     dx = x - x0
+    scale = 1.0 if n_gpu is None else math.sqrt(x.size / n_gpu)
     checks = [("mean_x", x.mean(), se_mean(x)), ("mean_v", v.mean(), se_mean(v)),
               ("mean_e", e.mean(), se_mean(e)), ("var_x", x.var(), se_var(x)),
               ("var_v", v.var(), se_var(v)), ("mean_dx", dx.mean(), se_mean(dx)),
               ("mean_dx2", (dx * dx).mean(), se_mean(dx * dx)), ("mean_x2", (x * x).mean(), se_mean(x * x))]
     for key, want, se in checks:
         g = float(got[key])
+        se *= scale
         tol = 3.0 * se + 1e-4 * abs(want)
-        print(f"{name} {key}: gpu {g:+.6f} oracle-subset {want:+.6f} +- {se:.6f}")
+        print(f"{name} {key}: gpu {g:+.6f} oracle sample {want:+.6f}, SE {se:.6f}, deviation {abs(g - want) / se:.2f} SE")
         assert abs(g - want) <= tol, (name, key, g, want, se)
 
 
 def test_config0_full_run_moments(abm, oracle):
-    """config[0] in full on both sides: 4,096 particles x 10,000 steps, <v>, <x>, var(x) at end."""
+    """config[0] in full on both sides: 4,096 particles x 10,000 steps, <v>, <x>, var(x) (and the other moments)
+    at the end, the SAME trajectories in the oracle.  Single trajectories decorrelate from their fp64 twins over
+    10^4 steps (fp32 rounding is amplified by the dynamics), so the ensembles are compared: 3 SE + 1e-4 relative.
+    Both sides see the same noise, so the two ensembles fluctuate together and the bar is met with a wide margin
+    (deviations of 0.0 ... 0.3 SE).  An oracle sample of OTHER trajectories would not do here: config[0]'s own 4,096
+    trajectories (seed 42) sit 2.9 SE below the mean of 65,536 others in <x> and <dx> -- in the oracle as on the GPU
+    (<dx> = 0.0144 and 0.0148 against 0.054 +- 0.003): a property of that noise realisation, not of either side."""
     wl = W.config0()
     p = wl.set_params(0)
     with abm.Ensemble([p], wl.n_particles, wl.seed) as ens:
@@ -509,8 +521,6 @@ def test_config0_full_run_moments(abm, oracle):
         st = ens.state()
     want = oracle_states(oracle, p, wl.seed, np.arange(wl.n_particles), wl.n_steps)
     x0 = oracle.init_many(p, wl.seed, wl.n_particles)[0]
-    # Same indices on both sides.  Single trajectories decorrelate over 10^4 steps (fp32 rounding
-    # is amplified by the dynamics), so they are compared as ensembles: 3 SE + 1e-4 relative.
     _moment_check("cfg0", m, want, x0)
     assert np.isfinite(st).all() and np.abs(st[:, 0]).max() < 50
 
@@ -537,26 +547,32 @@ def test_full_run_moments_vs_oracle_subset(abm, oracle, name, mk, every):
 
 
 def test_config2_sweep_moments_vs_oracle_subgrid(abm, oracle):
-    """config[2] at full size; the oracle integrates a 6 x 6 sub-grid of parameter sets (all 64
-    realisations each) for the full 10,000 steps: per-set <v>, var(v)."""
+    """config[2] at full size: per-set <v>, var(v) (and <e>) of the GPU's 64 realisations against the oracle on a
+    6 x 6 sub-grid of parameter sets, full 10,000 steps.  64 realisations fix a moment only to its own standard
+    error, and the GPU's fp32 trajectories decorrelate from their fp64 twins, so the oracle integrates 1,024 OTHER
+    realisations of each picked set (trajectory indices beyond the sweep's), which fixes the set's moments to a
+    quarter of that; every one of the 108 checks is then asserted at 3 SE (of a 64-realisation ensemble) + 1e-4
+    relative, strictly."""
     wl = W.config2()
     sets = [wl.set_params(s) for s in range(wl.n_param_sets)]
     with abm.Ensemble(sets, wl.n_particles, wl.seed) as ens:
         ens.step(wl.n_steps)
         m = ens.moments()
     pick = [256 * i + j for i in (0, 51, 102, 153, 204, 255) for j in (0, 51, 102, 153, 204, 255)]
-    n_fail = 0
+    n_orc = 1024
+    worst = 0.0
     for s in pick:
-        idx = np.arange(s * wl.n_particles, (s + 1) * wl.n_particles)
+        idx = wl.n_trajectories + s * n_orc + np.arange(n_orc)      # independent of the GPU's trajectories
         sub = oracle_states(oracle, sets[s], wl.seed, idx, wl.n_steps)
-        v = sub[:, 1]
-        # same 64 trajectories on both sides; 64 samples make wide error bars, so also count
+        v, e = sub[:, 1], sub[:, 2]
+        scale = math.sqrt(n_orc / wl.n_particles)
         for key, want, se in [("mean_v", v.mean(), se_mean(v)), ("var_v", v.var(), se_var(v)),
-                              ("mean_e", sub[:, 2].mean(), se_mean(sub[:, 2]))]:
-            ok = abs(float(m[key][s]) - want) <= 3.0 * se + 1e-4 * abs(want)
-            n_fail += not ok
-            assert abs(float(m[key][s]) - want) <= 5.0 * se + 1e-3 * abs(want) + 1e-9, (s, key)
-    assert n_fail <= 2, n_fail            # 108 checks at 3 SE: expect ~0.3 excursions
+                              ("mean_e", e.mean(), se_mean(e))]:
+            se *= scale
+            dev = abs(float(m[key][s]) - want)
+            worst = max(worst, dev / (3.0 * se + 1e-4 * abs(want) + 1e-300))
+            assert dev <= 3.0 * se + 1e-4 * abs(want), (s, key, float(m[key][s]), want, se)
+    print(f"cfg2: worst deviation {worst:.2f} of the bar (3 SE + 1e-4 relative) over {3 * len(pick)} checks")
     # the q = 0 column is a passive particle: no current, whatever D (pin P8 on the GPU)
     col0 = m["mean_v"][0::256]
     assert abs(col0.mean()) < 4.0 * np.sqrt(np.mean(m["var_v"][0::256]) / (64 * 256))
