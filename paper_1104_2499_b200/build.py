@@ -49,9 +49,10 @@ PIPE_RATES_EXE = os.path.join(PKG, "pipe_rates")
 def build_pipe_rates(force: bool = False) -> str:
     """The stand-alone issue-rate diagnostic (csrc/pipe_rates.cu): not needed by the library."""
     if not force and os.path.exists(PIPE_RATES_EXE) and \
-            os.path.getmtime(PIPE_RATES_EXE) >= os.path.getmtime(PIPE_RATES_SRC):
+            os.path.getmtime(PIPE_RATES_EXE) >= max(os.path.getmtime(PIPE_RATES_SRC),
+                                                    os.path.getmtime(os.path.join(CSRC, "abm_device.cuh"))):
         return PIPE_RATES_EXE
-    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+    cmd = [nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-I", CSRC,
            "-o", PIPE_RATES_EXE, PIPE_RATES_SRC]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:

@@ -12,9 +12,11 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
 #include <vector>
 #include <algorithm>
 #include <cuda_runtime.h>
+#include "abm_device.cuh"  // only for the last table: the accuracy of box_muller_f32 as the step kernels call it
 
 #define CK(x)                                                                      \
   do {                                                                             \
@@ -544,6 +546,48 @@ void chain_row(const Dev& d) {
   std::printf("%-72s %8.2f\n", CHAIN_NAME[CH], static_cast<double>(c) / iters / 16);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Seventh table: accuracy of the fast fp32 Box-Muller (abm_device.cuh: box_muller_f32, MUFU.LG2 / SQRT / COS /
+// SIN) over ALL 2^23 values each uniform can take, against fp64 (sigma = 1).  lg2.approx is accurate to 2^-22
+// absolutely, so the radius rho = sqrt(-2 ln u1) loses relative accuracy as u1 -> 1; DESIGN.md 7 quotes these rows.
+// ---------------------------------------------------------------------------------------------
+__device__ unsigned long long g_bm[6];  // bit patterns of non-negative doubles: max-reduce as integers
+__global__ void bm_accuracy_kernel() {
+  const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;  // 23-bit uniform index
+  const uint32_t w = k << 9;
+  const float s2 = static_cast<float>(-2.0 * 0.6931471805599453);   // sigma = 1
+  const float bm_o = static_cast<float>(2.0 * 3.141592653589793 * 0x1p-24 - 3.0 * 3.141592653589793);
+  const abm::Normal2f z = abm::box_muller_f32(w, w, s2, bm_o);
+  const double u = (static_cast<double>(k) + 0.5) * 0x1p-23;
+  const double rho = sqrt(-2.0 * log(u));
+  const double e_rho = fabs(static_cast<double>(z.rho) - rho);
+  // Normal2f carries -cos, -sin of 2 pi u (NEGATED)
+  const double e_cs = fabs(-static_cast<double>(z.cs) - cospi(2.0 * u));
+  const double e_sn = fabs(-static_cast<double>(z.sn) - sinpi(2.0 * u));
+  const bool finite = isfinite(z.rho) && isfinite(z.cs) && isfinite(z.sn);
+  atomicMax(&g_bm[0], static_cast<unsigned long long>(__double_as_longlong(e_rho)));
+  atomicMax(&g_bm[1], static_cast<unsigned long long>(__double_as_longlong(e_rho / rho)));
+  atomicMax(&g_bm[2], static_cast<unsigned long long>(__double_as_longlong(e_cs)));
+  atomicMax(&g_bm[3], static_cast<unsigned long long>(__double_as_longlong(e_sn)));
+  if (!finite) atomicAdd(&g_bm[4], 1ull);
+  if (e_rho > 1e-5) atomicMax(&g_bm[5], static_cast<unsigned long long>(__double_as_longlong(1.0 - u)));
+}
+static void bm_accuracy_table() {
+  unsigned long long h[6] = {0, 0, 0, 0, 0, 0};
+  CK(cudaMemcpyToSymbol(g_bm, h, sizeof(h)));
+  bm_accuracy_kernel<<<(1u << 23) / 256, 256>>>();
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpyFromSymbol(h, g_bm, sizeof(h)));
+  auto d = [&](int i) { double v; memcpy(&v, &h[i], 8); return v; };
+  std::printf("# fast fp32 Box-Muller (box_muller_f32, sigma = 1) over all 2^23 uniforms, against fp64\n");
+  std::printf("%-72s %10.3e\n", "max |rho - sqrt(-2 ln u1)|", d(0));
+  std::printf("%-72s %10.3e\n", "max relative error of rho", d(1));
+  std::printf("%-72s %10.3e\n", "largest 1 - u1 with an absolute error of rho above 1e-5", d(5));
+  std::printf("%-72s %10.3e\n", "max |cos| error", d(2));
+  std::printf("%-72s %10.3e\n", "max |sin| error", d(3));
+  std::printf("%-72s %10llu\n", "non-finite results", h[4]);
+}
+
 int main() {
   Dev d;
   cudaDeviceProp p;
@@ -638,5 +682,6 @@ int main() {
   std::printf("# dependent-issue latency: one warp, one chain; SM cycles per link\n");
   chain_row<CH_FFMA>(d); chain_row<CH_FMUL>(d); chain_row<CH_COS>(d); chain_row<CH_FORCE>(d);
   chain_row<CH_EMSTEP>(d); chain_row<CH_EMSTEP2>(d); chain_row<CH_DFMA>(d); chain_row<CH_IMADW>(d); chain_row<CH_LOP3>(d); chain_row<CH_LDS>(d);
+  bm_accuracy_table();
   return 0;
 }

@@ -8,8 +8,9 @@ scaling       PAPER.md:100-136 (Figs. 3-4): time of one launch against the numbe
               0, 10^3 and 10^4 iterations per launch; 20 launches per size, the last 15 averaged (:100);
               per-iteration time and offset from a linear fit over the iteration counts (:174).  Work items =
               trajectories of the paper's F0 sweep (one per parameter set, :74).  Sizes: powers of two
-              2^0 .. 2^22, and a fine sweep in steps of one eighth of a wave that shows where the paper's
-              "bands" (:122-134) fall on 148 SMs.
+              2^0 .. 2^22; the paper's own fine sweep, 50 .. 3,500 work items in steps of 50 (:122, Fig. 4), which on
+              148 SMs lies inside the flat region; and a fine sweep in steps of one eighth of a wave that shows
+              where the paper's "bands" (:122-134) would fall on this machine.
 presentation  PAPER.md:138-194 (Tab. 1): what showing a frame costs, in "iterations lost" = cost / time of
               one iteration at that size.  No graphics stack exists on this box, so the three columns are:
               the device-resident frame (the shared-buffer analogue, :156-162), a device->host copy of the
@@ -75,9 +76,10 @@ def scaling(out):
     sizes = [2 ** k for k in range(0, 23)]
     wave = 148 * 128 * 8                 # trajectories resident at once (one-set fp32 EM kernel: 8 CTAs/SM)
     fine = [wave * j // 8 for j in range(1, 33)]   # realisations of ONE parameter set (config[1]'s model)
+    paper_fine = list(range(50, 3501, 50))         # "from 50 to 3500 with step 50"
     rows = []
     with torch.cuda.stream(stream):
-        for kind, ns in (("pow2", sizes), ("fine", fine)):
+        for kind, ns in (("pow2", sizes), ("paper_fine", paper_fine), ("fine", fine)):
             for n in ns:
                 if kind == "fine":
                     n_eff = n
@@ -93,7 +95,7 @@ def scaling(out):
                         continue
                     t[it] = _launch_times(torch, ens, stream, it)
                 ens.close()
-                if kind == "pow2":
+                if kind != "fine":
                     xs = np.array([max(i, 1) for i in iters], float)
                     ys = np.array([t[i][0] for i in iters])
                     slope, offset = np.polyfit(xs, ys, 1)

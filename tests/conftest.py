@@ -10,6 +10,17 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    config.addinivalue_line("markers", "soak: long randomised runs, opt-in: -m 'gpu and soak' (skipped otherwise)")
+
+
+def pytest_collection_modifyitems(config, items):
+    # soak tests run only when the marker expression names them
+    if "soak" in (config.getoption("-m") or ""):
+        return
+    skip = pytest.mark.skip(reason="opt-in: -m 'gpu and soak'")
+    for item in items:
+        if "soak" in item.keywords:
+            item.add_marker(skip)
 
 
 @pytest.fixture(scope="session")

@@ -7,6 +7,7 @@ Tolerances (BASELINE.json north_star; readings in DESIGN.md):
   * abm_step(a); abm_step(b) == abm_step(a + b), snapshots, reductions: bit-exact / 1e-12
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -872,8 +873,9 @@ def test_tilt_table_across_launch_chunks(abm):
 # randomised differential test: random (seeded) models, sizes, launch splits and frame periods
 # ---------------------------------------------------------------------------------------------
 
-@pytest.mark.parametrize("case", range(64))
-def test_random_cases_against_the_oracle(abm, torch, oracle, case):
+def _random_case(abm, torch, oracle, case):
+    """One seeded random model / size / launch split / frame period against the oracle.  -> (worst error / bound,
+    whether the library itself flags the ensemble as beyond what its fp32 mode promises)."""
     rng = np.random.default_rng(9000 + case)
     precision = int(rng.integers(0, 2))
     n_sets = int(rng.choice([1, 1, 2, 5]))
@@ -894,6 +896,7 @@ def test_random_cases_against_the_oracle(abm, torch, oracle, case):
     total = sum(splits)
     with abm.Ensemble(sets, n, seed, snapshot_every=K, traj_base=base_idx, accuracy=acc) as ens, \
             abm.Ensemble(sets, n, seed, traj_base=base_idx, accuracy=acc) as ref:
+        beyond = bool(ens.beyond_tolerance)
         frame = ens.bind_snapshot(with_e=bool(rng.integers(0, 2))) if K else None
         for part in splits:
             ens.step(part)
@@ -915,6 +918,7 @@ def test_random_cases_against_the_oracle(abm, torch, oracle, case):
         # dt max|U''|; AUTO switches above 0.15): the bound is scaled by how far beyond that the set is
         stiff = max(p["dt"] * (2 * math.pi / p["L"])**2 * (abs(p["A1"]) + 4 * abs(p["A2"])) for p in sets)
         tol *= max(1.0, stiff / 0.15)
+    worst = 0.0
     for s, p in enumerate(sets):
         first = base_idx + s * n
         x, v, e = oracle.init_many(p, seed, n, first)
@@ -925,11 +929,38 @@ def test_random_cases_against_the_oracle(abm, torch, oracle, case):
             err = scale_rel_err(got[s], want)
         else:                                  # too few trajectories for an RMS scale: absolute, scale 1
             err = np.abs(got[s] - want).max(0) / np.maximum(1.0, np.abs(want).max(0))
-        assert np.all(err <= tol), (case, s, err, dict(base, **p))
+        worst = max(worst, float(np.max(err / tol)))
+        if not beyond:
+            assert np.all(err <= tol), (case, s, err, dict(base, **p))
         x0f = x0.astype(np.float32).astype(np.float64) if precision == 0 else x0
         om = oracle.moments(got[s][:, 0].copy(), got[s][:, 1].copy(), got[s][:, 2].copy(), x0f)
         for k_, val in om.items():
             assert m[k_][s] == pytest.approx(val, rel=1e-8, abs=1e-10), (case, s, k_)
+    return worst, beyond
+
+
+@pytest.mark.parametrize("case", range(64))
+def test_random_cases_against_the_oracle(abm, torch, oracle, case):
+    worst, beyond = _random_case(abm, torch, oracle, case)
+    # the 64 committed cases all pass the bound, flagged or not (cases the library flags as beyond what its fp32
+    # mode promises -- include/abm.h, ABM_ACCURACY_BEYOND_TOLERANCE -- are only reported by the soak below)
+    assert worst <= 1.0, (case, worst, beyond)
+
+
+@pytest.mark.soak
+def test_random_cases_soak(abm, torch, oracle):
+    """Opt-in soak (`-m "gpu and soak"`, ABM_SOAK_CASES=N, default 2,000): N more cases of the generator above.
+    Every invariant (split launches, frames, moments) is asserted in each case; the parity bound is asserted for
+    every ensemble the library does not itself flag as beyond what its fp32 mode promises, and the flagged ones
+    that exceed it are counted and printed."""
+    n_cases = int(os.environ.get("ABM_SOAK_CASES", "2000"))
+    flagged_over = []
+    for case in range(64, 64 + n_cases):
+        worst, beyond = _random_case(abm, torch, oracle, case)
+        if worst > 1.0:
+            assert beyond, (case, worst)
+            flagged_over.append((case, round(worst, 2)))
+    print(f"soak: {n_cases} random cases; flagged as beyond tolerance and over the bound: {flagged_over}")
 
 
 # ---------------------------------------------------------------------------------------------
@@ -1039,6 +1070,42 @@ def test_small_ensemble_kernel_is_bit_identical(abm, torch, monkeypatch, step_ke
     assert np.array_equal(a[1].view(np.uint8), b[1].view(np.uint8))
     if K:
         assert np.array_equal(a[2], b[2])
+
+
+@pytest.mark.soak
+def test_small_ensemble_kernel_soak(abm, torch, step_kernel_choice):
+    """Opt-in soak (`-m "gpu and soak"`, ABM_SOAK_CASES=N, default 2,000): step_kernel_small against step_kernel on
+    N seeded random models, sizes up to 8,192, frame periods and launch splits -- state, moments and frames bit for bit."""
+    if step_kernel_choice != "auto":
+        pytest.skip("compares both kernels itself")
+    n_cases = int(os.environ.get("ABM_SOAK_CASES", "2000"))
+    for case in range(n_cases):
+        rng = np.random.default_rng(77000 + case)
+        n_sets = int(rng.choice([1, 1, 1, 3, 17]))
+        base = dict(W.DEFAULTS, integrator=int(rng.integers(0, 2)), dt=float(rng.choice([1e-3, 5e-3])),
+                    A=float(rng.choice([0.0, 0.5])), omega=float(rng.uniform(0.3, 2.0)))
+        sets = [dict(base, D=float(rng.uniform(0.0, 0.3)), q=float(rng.uniform(0.0, 2.0)),
+                     F0=float(rng.uniform(-0.5, 0.5)), A1=float(rng.uniform(-1.0, 1.0)),
+                     L=float(rng.choice([0.5, 1.0]))) for _ in range(n_sets)]
+        n = int(rng.integers(1, max(8192 // n_sets, 2)))
+        K = int(rng.choice([0, 4, 8, 12, 100]))
+        acc = int(rng.integers(0, 3))
+        splits = [int(t) for t in rng.integers(1, 300, size=int(rng.integers(1, 4)))]
+        got = []
+        for choice in (abm.ABM_STEP_KERNEL_PER_THREAD, abm.ABM_STEP_KERNEL_SPLIT_WARPS):
+            with abm.Ensemble(sets, n, 1000 + case, snapshot_every=K, accuracy=acc, step_kernel=choice) as ens:
+                frame = ens.bind_snapshot(with_e=True) if K else None
+                for part in splits:
+                    ens.step(part)
+                st, m = ens.state(), ens.moments()
+                torch.cuda.synchronize()
+                got.append((st, m.copy(), None if frame is None else frame.cpu().numpy()))
+        a, b = got
+        assert np.array_equal(a[0], b[0]), case
+        assert np.array_equal(a[1].view(np.uint8), b[1].view(np.uint8)), case
+        if K:
+            assert np.array_equal(a[2], b[2]), case
+    print(f"soak: {n_cases} random cases, step_kernel_small == step_kernel bit for bit")
 
 
 def test_more_than_2_to_31_trajectories(abm, torch, oracle, step_kernel_choice):
