@@ -58,12 +58,20 @@ LANES_FP64 = 64
 # Each entry carries the git blob ids of the two kernel sources it was captured on: when a source has changed
 # since, the figures are stale and the line says null instead (re-capture, then update the entry).
 # The frame (one, overwritten) and the state stay in the 126 MB L2 during a launch, so the traffic is far BELOW
-# the algorithmic bytes.  configs[2-4] were captured on launches shortened with --sim-steps; a launch reads the
-# state once and writes it once whatever its step count, so the traffic figure holds, and the executed count per
-# particle-step is that of the loop.
+# the algorithmic bytes.  Every capture is of the full launch bench.py times (config[3]: one of the 20 launches of
+# 1,000 steps a pass is made of).
+_SRC = dict(kernels="0de9475028dab8808e94983a210a9710ec9535ff", device="06fe9e9ccfc6a44b54143a1038a941dd9225e44e",
+            summary="profiles/r02_step_kernels_ncu_full.md")
 NCU_CAPTURE = {
     # cfg: dict(traffic=bytes per launch, executed=per particle-step, kernels=blob of csrc/abm_kernels.cuh,
     #           device=blob of csrc/abm_device.cuh, summary=file under profiles/)
+    0: dict(traffic=79_872, executed=39.23, **_SRC),
+    1: dict(traffic=12_652_032, executed=29.15, **_SRC),
+    2: dict(traffic=57_197_568, executed=28.54, **_SRC),
+    # one of the 20 launches (1,000 steps each) of a pass
+    3: dict(traffic=21_008_640, executed=48.86, **_SRC),
+    # FP64-pipe operations (146 per Philox block in the loop; ncu: sm__pipe_fp64_cycles_active 71.55 %)
+    4: dict(traffic=156_946_176, executed=36.5, **_SRC),
 }
 # Warp-lane instructions per particle-step of the xorshift variant are not frozen anywhere: no `frac` for it.
 

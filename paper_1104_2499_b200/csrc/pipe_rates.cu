@@ -428,7 +428,7 @@ __global__ void __launch_bounds__(128) f64_mix_kernel(int iters, const float* __
       if (MODE & 1) { PR_DF(d[2]) PR_DF(d[3]) PR_DF(d[4]) PR_DF(d[5]) PR_DM(d[6]) PR_DF(d[7]) PR_DF(d[8]) PR_DF(d[9]) PR_DM(d[10]) PR_DA(d[11]) }
       if (MODE & 2) { PR_IW(u[2]) PR_IW(u[3]) }
       if (MODE & 4) { PR_ID(cv[2], u[6]) }
-      if (MODE & 16) { PR_IM(u[7]) PR_IM(u[4]) PR_IM(u[5]) PR_IM(u[6]) }
+      if (MODE & (16 | 64)) { PR_IM(u[7]) PR_IM(u[4]) PR_IM(u[5]) PR_IM(u[6]) }  // 64: only these 4 (8 per block)
       if (MODE & 8) { PR_LX(u[7]) PR_LX(u[4]) PR_LX(u[5]) PR_LX(u[6]) PR_LX(u[7]) }
       if (MODE & 1) {
         PR_DF(d[0]) PR_DF(d[1]) PR_DF(d[2]) PR_DF(d[3]) PR_DM(d[4]) PR_DF(d[5]) PR_DF(d[6]) PR_DF(d[7]) PR_DM(d[8]) PR_DA(d[9])
@@ -678,6 +678,7 @@ int main() {
   ROW(f64_mix, 19, "FP64 + Philox + 20 IMAD")
   ROW(f64_mix, 63, "all (the fp64 loop's mix, 257 instructions)")
   ROW(f64_mix, 47, "all but the 20 IMAD")
+  ROW(f64_mix, 111, "all with 8 IMAD instead of 20 (the loop of round 2: 227 instructions)")
 #undef ROW
   std::printf("# dependent-issue latency: one warp, one chain; SM cycles per link\n");
   chain_row<CH_FFMA>(d); chain_row<CH_FMUL>(d); chain_row<CH_COS>(d); chain_row<CH_FORCE>(d);
