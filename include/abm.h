@@ -42,8 +42,9 @@
  *   - A context belongs to the device that was current at abm_create.  Later calls may be made
  *     with any device current: the library switches to the context's device and restores the
  *     caller's before it returns.
- *   - Small fp32 ensembles (up to 8,192 trajectories) are integrated by a kernel that splits the work
- *     of a trajectory between warps (noise / integration) instead of one trajectory per thread; the
+ *   - Small fp32 ensembles (up to three 32-trajectory CTAs per SM: 14,208 trajectories on a B200) are
+ *     integrated by a kernel that splits the work of a trajectory between warps (noise /
+ *     integration) instead of one trajectory per thread; the
  *     results are bit-identical.  abm_params.step_kernel overrides the choice: a tuning and test knob,
  *     not part of the semantics.  The library reads no environment variable.
  *   - A handle is valid from a successful abm_create until abm_destroy.  Calls on a NULL, never

@@ -38,7 +38,7 @@ def torch():
 @pytest.fixture(autouse=True, params=["auto", "one_per_thread"])
 def step_kernel_choice(request, monkeypatch):
     """Every test runs twice: with the library's own choice between step_kernel_small (ensembles up to
-    8,192 trajectories, launches of whole Philox blocks) and step_kernel, and with step_kernel forced
+    14,208 trajectories, launches of whole Philox blocks) and step_kernel, and with step_kernel forced
     (abm_params.step_kernel = ABM_STEP_KERNEL_PER_THREAD in every record the binding builds) -- the small
     test ensembles would otherwise never reach the kernel the full-size configs run."""
     from paper_1104_2499_b200 import binding
@@ -1038,7 +1038,7 @@ def test_moments_async_matches_the_waiting_call(abm, torch):
 
 BOTH_KERNELS = [
     ("cfg0", W.config0, 4096, None, 0, 1000), ("cfg0_ragged", W.config0, 1000, None, 0, 264),
-    ("cfg0_8192", W.config0, 8192, None, 0, 64), ("cfg1_K100", W.config1, 700, None, 100, 1000),
+    ("cfg0_8192", W.config0, 8192, None, 0, 64), ("cfg0_14208", W.config0, 14208, None, 8, 64), ("cfg1_K100", W.config1, 700, None, 100, 1000),
     ("cfg1_K8", W.config1, 33, None, 8, 200), ("cfg3", W.config3, 777, None, 0, 400),
     ("cfg3_K4", W.config3, 100, None, 4, 64), ("cfg2_sets", W.config2, 64, 24, 0, 300),
     ("cfg2_sets_K12", W.config2, 5, 100, 12, 120), ("one_trajectory", W.config0, 1, None, 4, 4000),
