@@ -419,7 +419,9 @@ def run_ours(args, wl, cfg_id):
         philox = args.rng == "philox"
         out["roofline"] = {
             "bound": "alu",
-            "kernel": "abm::step_kernel_small" if (not fp64 and args.rng == "philox" and T <= 8192) else "abm::step_kernel",
+            "kernel": "abm::step_kernel_small" if (not fp64 and args.rng == "philox" and
+                                                    T <= 96 * torch.cuda.get_device_properties(0).multi_processor_count)
+            else "abm::step_kernel",   # AUTO: up to three 32-trajectory CTAs per SM (include/abm.h)
             "achieved": achieved / 1e12 if philox else None,
             "peak": peak / 1e12,
             "unit": "Tinstr/s (FP64-pipe lane operations)" if fp64 else "Tinstr/s (warp-lane instructions)",
