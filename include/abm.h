@@ -69,7 +69,9 @@ typedef enum abm_status {
                       non-finite or non-positive dt / L / gamma0 (when init_v = 1)             */
   ABM_ENOMEM = -2, /* device or host allocation failed                                        */
   ABM_ECUDA = -3,  /* CUDA error (sticky: reported by this and every later call)              */
-  ABM_ESTATE = -4  /* null or destroyed context                                               */
+  ABM_ESTATE = -4, /* null or destroyed context                                               */
+  ABM_ELIMIT = -5  /* the job needs more of the library's fixed, built-in scratch than exists
+                      (abm_frame_moment_sums_static only; nothing was launched)                */
 } abm_status;
 
 enum { ABM_FP32 = 0, ABM_FP64 = 1 };               /* abm_params.precision  */
@@ -205,6 +207,57 @@ int abm_moment_sums(abm_ctx* ctx, double* out);
 int abm_moment_sums_dev(abm_ctx* ctx, double* dev_out);
 int abm_moments_from_sums(const double* sums, uint32_t n_param_sets, uint64_t step,
                           abm_moment* out_moments);
+
+/* The moment sums of a FRAME, for callers that must not allocate device memory.
+ *
+ * Who this is for.  Every other reduction above works on a context, and abm_create takes the context's
+ * state and its reduction scratch from the CUDA allocator.  Some programs cannot do that at the point
+ * where they want the moments: a host application that hands this library a fixed memory budget and owns
+ * every device allocation itself (the frame then lives in ITS buffer, e.g. a tensor of its framework's
+ * caching allocator, which cannot see memory a library takes behind its back); a service that has pinned
+ * all of the GPU's memory up front; a latency-critical loop in which cudaMalloc / cudaFree -- which may
+ * take driver locks and synchronise the whole device -- are forbidden after start-up.  Such a caller
+ * passes the frame it already holds and a place for the result; this function calls no cudaMalloc,
+ * cudaFree, pool or any other allocating routine, neither on the host nor on the device.
+ *
+ * What it computes.  The same eight sums per parameter set as abm_moment_sums_dev, in the same order of
+ * additions (so the results are bit-identical to that call on the same state):
+ *   dev_out[s][0..7] = { N, sum x, sum x^2, sum v, sum v^2, sum e, sum dx, sum dx^2 },  dx = x - x(0)
+ * over the n_particles trajectories of set s, which occupy rows [s n_particles, (s + 1) n_particles).
+ *   dev_frame   DEVICE, read only: a frame as abm_snapshot writes it -- fp32: stride 8 (x, v) or 16
+ *               (x, v, e, 1); fp64: stride 16 or 32 -- aligned to stride_bytes.  With the short stride
+ *               there is no e: sum e is 0.
+ *   dev_frame0  DEVICE, read only, or NULL: a frame of the same layout taken at step 0; its x column is
+ *               x(0).  NULL: sum dx = sum dx^2 = 0.
+ *   dev_out     DEVICE, 8-byte aligned, [n_param_sets][ABM_N_SUMS] doubles, overwritten.  Feed a host copy
+ *               to abm_moments_from_sums for means and variances.
+ *   precision   ABM_FP32 | ABM_FP64 (the element type of the frames);  stream: cudaStream_t or NULL.
+ * Asynchronous on `stream`; the caller keeps ownership of all three buffers.
+ *
+ * The scratch.  The per-CTA partial sums go into an array that is part of the library image itself (a
+ * file-scope __device__ array, ABM_STATIC_SCRATCH_BYTES = 3.5 MiB).  Every GPU on which the library's code is
+ * loaded holds that array from load until the process exits, whether or not this function is ever called.
+ * It has room for ABM_STATIC_MAX_SLICES partial records; a set needs ceil(n_particles / 4096) of them (one
+ * when n_particles <= 4096), so the limit is  n_param_sets * ceil(n_particles / 4096) <= 65,536  -- e.g. one
+ * set of 268 million trajectories, or BASELINE.json's sweep of 65,536 sets x 64.  Beyond it the call
+ * returns ABM_ELIMIT and launches nothing.
+ *
+ * Rules that follow from one shared array:
+ *   - Calls whose kernels may run at the same time on one GPU (different streams, several host threads)
+ *     write the same partial records and corrupt each other's sums.  Put them on one stream, or order
+ *     them with events.  (Calls on different GPUs do not interfere: each GPU has its own copy.)
+ *   - The array keeps what the previous call left in it.  Nothing here depends on that: every record a
+ *     call reads back has been written by that same call first, so no clearing is needed or done.
+ *   - The first call on each GPU looks up the array's device address (cudaGetSymbolAddress, with that GPU
+ *     current; the result is cached per device).  Make that first call during start-up, outside any
+ *     stream capture.
+ * Errors: ABM_EINVAL (null / misaligned pointer, zero counts, bad stride or precision), ABM_ELIMIT,
+ * ABM_ECUDA (no device, address lookup or launch failed). */
+#define ABM_STATIC_MAX_SLICES 65536u
+#define ABM_STATIC_SCRATCH_BYTES (ABM_STATIC_MAX_SLICES * 7u * 8u)
+int abm_frame_moment_sums_static(const void* dev_frame, const void* dev_frame0, size_t stride_bytes,
+                                 uint32_t precision, uint64_t n_particles, uint32_t n_param_sets,
+                                 double* dev_out, void* stream);
 
 /* The quantity the paper plots (Fig. 2: mean velocity against the load force, "over
  * time, results ... are averaged", :74): the velocity of each set averaged over its realisations AND

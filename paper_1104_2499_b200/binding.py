@@ -13,7 +13,7 @@ import numpy as np
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libabm_b200.so")
 
-ABM_OK, ABM_EINVAL, ABM_ENOMEM, ABM_ECUDA, ABM_ESTATE = 0, -1, -2, -3, -4
+ABM_OK, ABM_EINVAL, ABM_ENOMEM, ABM_ECUDA, ABM_ESTATE, ABM_ELIMIT = 0, -1, -2, -3, -4, -5
 ABM_FP32, ABM_FP64 = 0, 1
 ABM_EULER_MARUYAMA, ABM_HEUN = 0, 1
 ABM_ACCURACY_AUTO, ABM_ACCURACY_FAST, ABM_ACCURACY_PRECISE = 0, 1, 2
@@ -21,6 +21,7 @@ ABM_ACCURACY_BEYOND_TOLERANCE = 0x100
 ABM_RNG_PHILOX, ABM_RNG_XORSHIFT128 = 0, 1
 ABM_STEP_KERNEL_AUTO, ABM_STEP_KERNEL_PER_THREAD, ABM_STEP_KERNEL_SPLIT_WARPS = 0, 1, 2
 ABM_N_SUMS = 8
+ABM_STATIC_MAX_SLICES = 65536        # partial records in the built-in scratch of abm_frame_moment_sums_static
 
 # abm_params.step_kernel of records built by make_params when the caller names none.  The GPU tests flip it
 # to run every case through both step kernels (results are bit-identical whichever runs).
@@ -55,7 +56,7 @@ MOMENT_DTYPE = np.dtype([("n", "<u8"), ("step", "<u8"), ("mean_x", "<f8"), ("var
 
 EXPORTS = ["abm_create", "abm_step", "abm_snapshot", "abm_snapshot_host", "abm_moments", "abm_moments_async",
            "abm_moment_sums", "abm_moment_sums_dev", "abm_moments_from_sums", "abm_time_averaged_velocity",
-           "abm_raster", "abm_get_step", "abm_get_accuracy", "abm_destroy", "abm_trim", "abm_philox_blocks",
+           "abm_frame_moment_sums_static", "abm_raster", "abm_get_step", "abm_get_accuracy", "abm_destroy", "abm_trim", "abm_philox_blocks",
            "abm_philox_blocks_loop", "abm_strerror", "abm_abi_version"]
 
 _lib = None
@@ -87,6 +88,7 @@ def lib():
         L.abm_moment_sums_dev.argtypes = [vp, vp]
         L.abm_moments_from_sums.argtypes = [vp, u32, u64, vp]
         L.abm_time_averaged_velocity.argtypes = [vp, vp]
+        L.abm_frame_moment_sums_static.argtypes = [vp, vp, C.c_size_t, u32, u64, u32, vp, vp]
         L.abm_raster.argtypes = [vp, vp, u32, u32, C.c_double, C.c_double, vp, u32]
         L.abm_get_step.argtypes = [vp, C.POINTER(u64)]
         L.abm_get_accuracy.argtypes = [vp, C.POINTER(u32)]
@@ -187,6 +189,18 @@ def abm_moments_from_sums(sums, step):
     _check("abm_moments_from_sums",
            lib().abm_moments_from_sums(sums.ctypes.data, sums.shape[0], step, out.ctypes.data))
     return out
+
+
+def abm_frame_moment_sums_static(dev_frame, dev_frame0, stride_bytes, precision, n_particles, n_param_sets,
+                                 dev_out, stream=0):
+    """The eight moment sums per set of a caller-owned device frame, written to caller-owned device memory
+    [n_param_sets][8], without any device allocation by the library (its scratch is a fixed array inside the
+    library image: at most ABM_STATIC_MAX_SLICES slices of 4096 trajectories, else ABM_ELIMIT).  For
+    callers that own all device memory themselves or may not allocate once their loop runs.  Calls
+    share that scratch: keep them on one stream.  The first call per GPU belongs to start-up."""
+    _check("abm_frame_moment_sums_static",
+           lib().abm_frame_moment_sums_static(dev_frame, dev_frame0 or None, stride_bytes, precision, n_particles,
+                                              n_param_sets, dev_out, stream or None))
 
 
 def abm_time_averaged_velocity(ctx, n_param_sets):

@@ -982,6 +982,7 @@ const char* abm_strerror(int status) {
     case ABM_ENOMEM: return "out of memory";
     case ABM_ECUDA: return "CUDA error (no usable device, or a launch/copy failed)";
     case ABM_ESTATE: return "null or destroyed context";
+    case ABM_ELIMIT: return "job exceeds the library's fixed built-in scratch (abm_frame_moment_sums_static)";
     default: return "unknown status";
   }
 }
@@ -989,3 +990,173 @@ const char* abm_strerror(int status) {
 uint32_t abm_abi_version(void) { return 6; }
 
 }  // extern "C"
+
+// =================================================================================================
+// abm_frame_moment_sums_static -- the moment sums of a caller-owned frame, for callers that may not
+// allocate (include/abm.h says who they are).  Nothing in this section calls cudaMalloc, cudaFree, a
+// memory pool or any other allocating routine; the two-pass reduction's intermediate records live in
+// the file-scope array below, which belongs to the library image and therefore exists, once per GPU
+// that loads the image, from load to process exit.
+//
+// The array is shared by every call on a GPU.  It is never cleared: pass 1 writes records
+// [0, n_sets * blocks_per_set) in full and pass 2 reads exactly those, so stale contents of an
+// earlier, larger call are never looked at.  Two calls whose kernels overlap on one GPU would write the
+// same records -- the header tells callers to keep them on one stream.
+// =================================================================================================
+namespace {
+
+constexpr uint32_t STATIC_RECORD = N_SUMS - 1;  // doubles per partial record (N is not summed)
+static_assert(ABM_STATIC_SCRATCH_BYTES == ABM_STATIC_MAX_SLICES * STATIC_RECORD * sizeof(double),
+              "ABM_STATIC_SCRATCH_BYTES in include/abm.h is the size of g_static_partial");
+
+// In HOST code this name is only a handle for cudaGetSymbolAddress: it is not a device address and must
+// never be handed to a kernel as is.  static_scratch_for() below resolves it.
+static __device__ __align__(256) double g_static_partial[ABM_STATIC_MAX_SLICES * STATIC_RECORD];
+
+std::mutex g_static_mutex;
+double* g_static_ptr[MAX_DEVICES] = {};  // device address of g_static_partial, per GPU (null: not looked up yet)
+
+// Device address of the scratch on `device`, which must be the CURRENT device (the runtime resolves a
+// symbol for whichever GPU is current).  Looked up once per GPU, then served from the cache.
+cudaError_t static_scratch_for(int device, double** out) {
+  if (device < 0 || device >= MAX_DEVICES) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_ptr[device]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_partial);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    g_static_ptr[device] = static_cast<double*>(p);
+  }
+  *out = g_static_ptr[device];
+  return cudaSuccess;
+}
+
+template <typename Real> struct FrameVec;
+template <> struct FrameVec<float> { using V2 = float2; using V4 = float4; };
+template <> struct FrameVec<double> { using V2 = double2; using V4 = double4; };
+
+// Pass 1, the frame-reading twin of moments_partial_kernel: same grid (one CTA per slice of a set), same
+// per-thread stride, same shuffle tree and same order over the warps, hence the same roundings.
+template <typename Real, bool WITH_E>
+__global__ void __launch_bounds__(MOM_BLOCK)
+frame_moments_partial_kernel(const void* __restrict__ frame, const void* __restrict__ frame0,
+                             uint64_t n_particles, uint32_t blocks_per_set, uint32_t slice,
+                             double* __restrict__ partial) {
+  using V2 = typename FrameVec<Real>::V2;
+  using V4 = typename FrameVec<Real>::V4;
+  const uint32_t set = blockIdx.x / blocks_per_set;
+  const uint32_t blk = blockIdx.x - set * blocks_per_set;
+  const uint64_t r0 = static_cast<uint64_t>(blk) * slice;
+  uint64_t r1 = r0 + slice;
+  if (r1 > n_particles) r1 = n_particles;
+  double acc[STATIC_RECORD] = {0, 0, 0, 0, 0, 0, 0};
+  for (uint64_t r = r0 + threadIdx.x; r < r1; r += blockDim.x) {
+    const uint64_t k = static_cast<uint64_t>(set) * n_particles + r;
+    double xi, vi, ei = 0.0, dx = 0.0;
+    if (WITH_E) {
+      const V4 s = static_cast<const V4*>(frame)[k];
+      xi = static_cast<double>(s.x), vi = static_cast<double>(s.y), ei = static_cast<double>(s.z);
+      if (frame0) dx = xi - static_cast<double>(static_cast<const V4*>(frame0)[k].x);
+    } else {
+      const V2 s = static_cast<const V2*>(frame)[k];
+      xi = static_cast<double>(s.x), vi = static_cast<double>(s.y);
+      if (frame0) dx = xi - static_cast<double>(static_cast<const V2*>(frame0)[k].x);
+    }
+    acc[0] += xi;
+    acc[1] += xi * xi;
+    acc[2] += vi;
+    acc[3] += vi * vi;
+    acc[4] += ei;
+    acc[5] += dx;
+    acc[6] += dx * dx;
+  }
+  __shared__ double sm[MOM_BLOCK / 32][STATIC_RECORD];
+  const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+#pragma unroll
+  for (uint32_t q = 0; q < STATIC_RECORD; ++q) {
+    double t = acc[q];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) t += __shfl_xor_sync(0xffffffffu, t, off);
+    if (lane == 0) sm[warp][q] = t;
+  }
+  __syncthreads();
+  if (threadIdx.x < STATIC_RECORD) {
+    double t = 0;
+    const uint32_t n_warps = (blockDim.x + 31u) >> 5;
+    for (uint32_t wq = 0; wq < n_warps; ++wq) t += sm[wq][threadIdx.x];
+    partial[static_cast<uint64_t>(blockIdx.x) * STATIC_RECORD + threadIdx.x] = t;
+  }
+}
+
+// Pass 2, moments_final_kernel without the finalised record: one warp per set adds that set's partial
+// records in the same fixed order and writes the eight sums straight into the caller's buffer.
+__global__ void __launch_bounds__(128)
+frame_moments_final_kernel(const double* __restrict__ partial, uint32_t n_sets, uint32_t blocks_per_set,
+                           uint64_t n_particles, double* __restrict__ sums) {
+  const uint32_t set = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const uint32_t lane = threadIdx.x & 31u;
+  if (set >= n_sets) return;  // whole warps leave together
+  double s[N_SUMS];
+  s[0] = static_cast<double>(n_particles);
+  const double* p = partial + static_cast<uint64_t>(set) * blocks_per_set * STATIC_RECORD;
+#pragma unroll
+  for (uint32_t q = 0; q < STATIC_RECORD; ++q) {
+    double t = 0;
+    for (uint32_t b = lane; b < blocks_per_set; b += 32) t += p[static_cast<uint64_t>(b) * STATIC_RECORD + q];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) t += __shfl_xor_sync(0xffffffffu, t, off);
+    s[q + 1] = t;
+  }
+  if (lane == 0)
+    for (int q = 0; q < N_SUMS; ++q) sums[static_cast<uint64_t>(set) * N_SUMS + q] = s[q];
+}
+
+}  // namespace
+
+extern "C" int abm_frame_moment_sums_static(const void* dev_frame, const void* dev_frame0, size_t stride_bytes,
+                                            uint32_t precision, uint64_t n_particles, uint32_t n_param_sets,
+                                            double* dev_out, void* stream) {
+  if (!dev_frame || !dev_out || n_particles == 0 || n_param_sets == 0 || precision > ABM_FP64)
+    return ABM_EINVAL;
+  const size_t real_size = precision == ABM_FP32 ? 4 : 8;
+  if (stride_bytes != 2 * real_size && stride_bytes != 4 * real_size) return ABM_EINVAL;
+  if (reinterpret_cast<uintptr_t>(dev_frame) % stride_bytes != 0 ||
+      reinterpret_cast<uintptr_t>(dev_frame0) % stride_bytes != 0 ||
+      reinterpret_cast<uintptr_t>(dev_out) % sizeof(double) != 0)
+    return ABM_EINVAL;
+  // the reduction geometry of abm_create, so that the sums come out bit-identical to a context's
+  uint32_t mb = MOM_BLOCK;
+  if (n_particles < MOM_BLOCK) mb = static_cast<uint32_t>((n_particles + 31) / 32 * 32);
+  const uint32_t slice = mb * MOM_PER_THREAD;
+  const uint64_t bps = (n_particles + slice - 1) / slice;
+  if (bps > ABM_STATIC_MAX_SLICES || bps * n_param_sets > ABM_STATIC_MAX_SLICES) return ABM_ELIMIT;
+  int device = -1;
+  if (cudaGetDevice(&device) != cudaSuccess) {  // no device: fail loudly, there is no CPU path
+    cudaGetLastError();
+    return ABM_ECUDA;
+  }
+  double* scratch = nullptr;  // the DEVICE address of g_static_partial on the current GPU
+  if (static_scratch_for(device, &scratch) != cudaSuccess) {
+    cudaGetLastError();
+    return ABM_ECUDA;
+  }
+  const cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const uint32_t grid = static_cast<uint32_t>(bps) * n_param_sets;
+  const uint32_t bpsu = static_cast<uint32_t>(bps);
+  const bool with_e = stride_bytes == 4 * real_size;
+  if (precision == ABM_FP32) {
+    if (with_e)
+      frame_moments_partial_kernel<float, true><<<grid, mb, 0, st>>>(dev_frame, dev_frame0, n_particles, bpsu, slice, scratch);
+    else
+      frame_moments_partial_kernel<float, false><<<grid, mb, 0, st>>>(dev_frame, dev_frame0, n_particles, bpsu, slice, scratch);
+  } else {
+    if (with_e)
+      frame_moments_partial_kernel<double, true><<<grid, mb, 0, st>>>(dev_frame, dev_frame0, n_particles, bpsu, slice, scratch);
+    else
+      frame_moments_partial_kernel<double, false><<<grid, mb, 0, st>>>(dev_frame, dev_frame0, n_particles, bpsu, slice, scratch);
+  }
+  if (cudaGetLastError() != cudaSuccess) return ABM_ECUDA;
+  frame_moments_final_kernel<<<(n_param_sets + 3) / 4, 128, 0, st>>>(scratch, n_param_sets, bpsu, n_particles, dev_out);
+  return cudaGetLastError() == cudaSuccess ? ABM_OK : ABM_ECUDA;
+}
