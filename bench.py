@@ -2,6 +2,7 @@
 """bench.py -- particle-steps/s of the hot path on BASELINE.json's config[1] (default), one JSON line.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+                    [--scaling weak|strong] [--all-configs PASSES]
 
 One bench "step" = one pass of the whole hot path over one batch of synthetic input
 (SURVEY.md 8(a) rows S0-S7): create + init the ensemble from its Philox init blocks, bind the
@@ -14,9 +15,15 @@ frame into pinned memory and of the moments.
 N > 1: one process per GPU.  Under torchrun (WORLD_SIZE set) this process is one rank; a bare
 `python bench.py --gpus N` re-executes itself under `python -m torch.distributed.run --nproc-per-node N`
 (127.0.0.1 rendezvous) and fails loudly if the box has fewer than N devices.  Each rank integrates its
-own shard of a N-times larger ensemble (weak scaling; trajectory indices rank*T ... via traj_base), and
-the only exchange is one all-reduce of the per-set raw moment sums (8 doubles per set) over NCCL on the
-device (sharding.MomentExchange: no host round trip), inside the timed region.
+own shard of a N-times larger ensemble (weak scaling, the default; trajectory indices rank*T ... via
+traj_base) or, with --scaling strong, its part [gT/G, (g+1)T/G) of the ONE ensemble (whole parameter sets
+per rank when there are at least N, else the realisations of every set divided), and the only exchange
+is one all-reduce of the per-set raw moment sums (8 doubles per set) over NCCL on the device
+(sharding.MomentExchange: no host round trip), inside the timed region.
+
+The default run (config 1, one GPU) then also times configs 0, 2, 3, 4 -- after the headline's timed regions,
+same protocol, 3 passes each -- and reports them under "all_configs" (value, kernel_ms, frac, frac_executed,
+e2e, clocks per config), so one driver-run line carries all five BASELINE.json configs.
 
 Timing protocol of the paper (PAPER.md:100 "20 steps ... last fifteen", :122 "average and standard
 deviation ... zero steps ... offset time"): besides the mean, the line carries the standard deviation over
@@ -252,6 +259,9 @@ def run_ours(args, wl, cfg_id):
     torch.cuda.set_device(local_rank % n_dev)
     if world > 1:
         if args.backend == "nccl":
+            # the communicator's own log lines (rank count, transport: NVLS / P2P over NVLink) go to stderr
+            os.environ.setdefault("NCCL_DEBUG", "INFO")
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
             dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
         else:   # gloo: exercises the multi-rank flow where ranks must share one GPU (NCCL refuses that)
             dist.init_process_group("gloo")
@@ -261,186 +271,213 @@ def run_ours(args, wl, cfg_id):
           file=sys.stderr, flush=True)
     abm.lib()
 
-    stream = torch.cuda.Stream()
-    sets = [dict(wl.set_params(s), rng=1 if args.rng == "xorshift" else 0) for s in range(wl.n_param_sets)]
-    T = wl.n_trajectories
-    # weak scaling: rank r integrates a full copy of the workload on global trajectories [r*T, (r+1)*T)
-    plan = sharding.shard_plan(wl.n_particles, wl.n_param_sets, rank, world, "weak")
-    traj_base = plan.traj_base
-    n_steps, M = wl.n_steps, (wl.moments_every or wl.n_steps)
-    fp64 = sets[0]["precision"] == 1
-    frame_cols = 2
-    frame_item = 8 if fp64 else 4
-    host_frame = torch.empty((T, frame_cols), dtype=torch.float64 if fp64 else torch.float32,
-                             pin_memory=True)
-    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")  # > 126 MB L2
-    (mom_out, _mom_keep), (sums_out, _sums_keep) = abm.pinned_moment_buffers(len(sets))  # pinned: true DMA
-    # one pinned record array per intermediate reduction of a pass (config[3]: 19)
-    mom_slots = [abm.pinned_moment_buffers(len(sets))[0] for _ in range(max(n_steps // M - 1, 0))]
-    # N > 1: device + pinned buffers of the one exchange, a slot per reduction of a pass
-    exchange = sharding.MomentExchange(plan, n_slots=n_steps // M, backend=args.backend) if world > 1 else None
-    launches = {"n": 0}
-    ens_tilt = any(p["A"] != 0.0 for p in sets)
-    step_launches = (2 if ens_tilt else 1) * -(-M // (65536 if ens_tilt else 2**30))
-    # parameter records marshalled once (host side); abm_create copies them to the device
-    params = abm.make_params(sets, stream=stream.cuda_stream, snapshot_every=wl.snapshot_every,
-                             traj_base=traj_base)
-    params_bytes = len(sets) * abm.C.sizeof(abm.abm_params)
-
-    def one_pass(e2e, ev=None):
-        """The whole hot path once.  Returns the moments (host)."""
-        with torch.cuda.stream(stream):
-            ens = abm.Ensemble(params, wl.n_particles, wl.seed, stream=stream)  # S0 (1 kernel)
-            launches["n"] += 1
-            if wl.snapshot_every:
-                ens.bind_snapshot()                                            # S5 (1 kernel)
-                launches["n"] += 1
-            m = None
-            for j in range(n_steps // M):
-                if ev is not None:
-                    ev[j][0].record(stream)
-                ens.step(M)                                                    # S1-S5, S7
-                if ev is not None:
-                    ev[j][1].record(stream)
-                launches["n"] += step_launches
-                if world > 1:                          # S6 (2 kernels) + all-reduce, enqueued: no host round trip
-                    exchange.enqueue(ens, j)
-                elif j + 1 < n_steps // M:     # intermediate reductions: enqueued, no host round trip
-                    ens.moments_async(mom_slots[j][0])                         # S6 (2 kernels)
-                else:                          # the last one waits: every record is on the host now
-                    m = ens.moments(mom_out)                                   # S6 (2 kernels)
-                launches["n"] += 2
-            if e2e:
-                abm.abm_snapshot_host(ens.ctx, host_frame.numpy(), frame_cols * frame_item)
-                launches["n"] += 1
-            ens.close()                                # waits for the stream: every record is on the host
-            if world > 1:
-                m = exchange.result(n_steps // M - 1)
-        return m
-
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 0)):
-        one_pass(False)
-        one_pass(True)
-    barrier()
-
-    # ---- device-timed arm -------------------------------------------------------------------
-    ev_pass = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-               for _ in range(args.steps)]
-    ev_kern = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-                for _ in range(n_steps // M)] for _ in range(args.steps)]   # around every abm_step
-    launches["n"] = 0
-    barrier()
-    wall0 = time.perf_counter()
-    with ClockSampler(torch.cuda.current_device()) as clk:
-        for i in range(args.steps):
-            flush.fill_(i & 0xff)                       # L2 flush between timed iterations
-            torch.cuda.synchronize()
-            ev_pass[i][0].record(stream)
-            m = one_pass(False, ev_kern[i])
-            ev_pass[i][1].record(stream)
-        barrier()
-    wall = time.perf_counter() - wall0
-    gpu_launches = launches["n"]
-    t_pass_ms = [a.elapsed_time(b) for a, b in ev_pass]
-    t_dev = sum(t_pass_ms) * 1e-3
-    t_kern_ms = [sum(a.elapsed_time(b) for a, b in evs) for evs in ev_kern]   # per pass, all abm_step calls
-
-    # ---- end-to-end arm (host params -> host frame + moments), wall clock ---------------------
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(args.steps):
-        m_e2e = one_pass(True)
-    barrier()
-    t_e2e = time.perf_counter() - t0
-
-    # ---- the paper's "offset time" (PAPER.md:122): 20 launches of one step, the last 15 (PAPER.md:100) ----
-    with torch.cuda.stream(stream):
-        ens = abm.Ensemble(params, wl.n_particles, wl.seed, stream=stream)
-        if wl.snapshot_every:
-            ens.bind_snapshot()
-        ev_off = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
-        for a, b in ev_off:
-            a.record(stream)
-            ens.step(1)
-            b.record(stream)
-        stream.synchronize()
-        ens.close()
-    t_off = [a.elapsed_time(b) for a, b in ev_off][5:]
-
-    tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=coll_dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    t_dev, t_e2e = float(tt[0]), float(tt[1])
-
-    psteps_job = wl.particle_steps * world * args.steps
-    value = psteps_job / t_dev
     peaks, peak_src = load_peaks()
     f_max = float(peaks.get("sm_max_mhz", 1965.0)) * 1e6
-    clocks = clk.summary()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")  # > 126 MB L2
 
-    out = {
-        "metric": "particle-steps/sec", "value": value, "unit": "particle-steps/s",
-        "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": 1e3 * t_dev / args.steps, "higher_is_better": True, "scaling": "weak",
-        "ms_per_step_sd": statistics.pstdev(t_pass_ms) if len(t_pass_ms) > 1 else None,   # this rank's passes
-        "offset_ms": {"mean": statistics.mean(t_off), "sd": statistics.pstdev(t_off),
-                      "protocol": "20 launches of 1 step, last 15 (PAPER.md:100, :122)"},
-        "vs_baseline": None,   # BASELINE.md: the paper states no throughput for this path
-        "dtype": "f64" if fp64 else "f32", "data": "synthetic",
-        "config": {"workload": wl.name, "baseline_config": cfg_id, "trajectories_per_gpu": T,
-                   "param_sets": wl.n_param_sets, "sim_steps": n_steps,
-                   "snapshot_every": wl.snapshot_every, "moments_every": M,
-                   "integrator": "heun" if sets[0]["integrator"] else "euler-maruyama", "rng": args.rng,
-                   "l2": "flushed between timed iterations (256 MiB fill)",
-                   "pass": "create+init, bind frame, integrate, moments, destroy"},
-        "e2e": {"value": psteps_job / t_e2e, "unit": "particle-steps/s",
-                "h2d_bytes_per_step": int(params_bytes),
-                "d2h_bytes_per_step": int(host_frame.numel() * host_frame.element_size()
-                                          + 80 * len(sets) * (n_steps // M)),
-                "timer": "wall clock, host parameter records -> pinned host frame + moments"},
-        "gpu_launches": gpu_launches,
-        "clocks": clocks,
-        "wall_s_timed_region": wall,
-    }
-    if t_kern_ms:
-        t_k = statistics.mean(t_kern_ms) * 1e-3
-        lane_instr = I_ALG[cfg_id] * wl.particle_steps
-        lanes = LANES_FP64 if fp64 else LANES_PER_SM
-        peak = N_SM * lanes * f_max
-        achieved = lane_instr / t_k
-        sm_mhz = clocks.get("sm_mhz") or (f_max / 1e6)
-        cap, cap_src = ncu_capture(cfg_id) if (not args.sim_steps and args.rng == "philox") else \
-            (None, "no capture of this launch (--sim-steps / --rng xorshift)")
-        philox = args.rng == "philox"
-        out["roofline"] = {
-            "bound": "alu",
-            "kernel": "abm::step_kernel_small" if (not fp64 and args.rng == "philox" and
-                                                    T <= 96 * torch.cuda.get_device_properties(0).multi_processor_count)
-            else "abm::step_kernel",   # AUTO: up to three 32-trajectory CTAs per SM (include/abm.h)
-            "achieved": achieved / 1e12 if philox else None,
-            "peak": peak / 1e12,
-            "unit": "Tinstr/s (FP64-pipe lane operations)" if fp64 else "Tinstr/s (warp-lane instructions)",
-            "frac": achieved / peak if philox else None,     # I_alg is frozen for the Philox path only
-            "frac_at_sustained_clock": achieved / (N_SM * lanes * sm_mhz * 1e6) if philox else None,
-            "i_alg_per_particle_step": I_ALG[cfg_id] if philox else None,
-            # the same with what the kernel executes per particle-step in place of I_alg (ncu capture): how busy
-            # the issue slots (fp64: the FP64 pipe) are, whatever the instructions are worth
-            "frac_executed": cap["executed"] * wl.particle_steps / t_k / peak if cap else None,
-            "executed_per_particle_step": cap["executed"] if cap else None,
-            "particle_steps_per_pass": wl.particle_steps,
-            "kernel_ms": 1e3 * t_k, "kernel_ms_sd": statistics.pstdev(t_kern_ms) if len(t_kern_ms) > 1 else None,
-            "kernel_launches_per_pass": step_launches * (n_steps // M),
-            "kernel_share_of_pass": sum(t_kern_ms) / sum(t_pass_ms),
-            "peak_source": f"148 SMs x {lanes} lanes x sm_max_mhz {f_max / 1e6:.0f} MHz, {peak_src}",
-            "traffic": cap["traffic"] if cap else None, "traffic_source": cap_src,
-            "hbm_algorithmic_bytes_per_launch": int(T * (24 + 8 * (n_steps // wl.snapshot_every
-                                                                   if wl.snapshot_every else 0))),
+    def measure(wl, cfg_id, steps, warmup, with_offset=True):
+        """`warmup` untimed + `steps` device-timed + `steps` end-to-end passes of one workload -> (line, moments)."""
+        stream = torch.cuda.Stream()
+        all_sets = [dict(wl.set_params(s), rng=1 if args.rng == "xorshift" else 0) for s in range(wl.n_param_sets)]
+        # weak: rank r integrates a full copy of the workload on global trajectories [r*T, (r+1)*T);
+        # strong: the one ensemble is divided (whole sets per rank, else realisations), SURVEY.md 8(e)
+        plan = sharding.shard_plan(wl.n_particles, wl.n_param_sets, rank, world, args.scaling)
+        sets = all_sets[plan.set_first:plan.set_first + plan.n_sets]
+        n_particles = plan.n_particles
+        T = n_particles * len(sets)                      # trajectories of THIS rank
+        n_steps, M = wl.n_steps, (wl.moments_every or wl.n_steps)
+        fp64 = sets[0]["precision"] == 1
+        frame_cols = 2
+        frame_item = 8 if fp64 else 4
+        host_frame = torch.empty((T, frame_cols), dtype=torch.float64 if fp64 else torch.float32,
+                                 pin_memory=True)
+        (mom_out, _mom_keep), (sums_out, _sums_keep) = abm.pinned_moment_buffers(len(sets))  # pinned: true DMA
+        # one pinned record array per intermediate reduction of a pass (config[3]: 19)
+        mom_slots = [abm.pinned_moment_buffers(len(sets))[0] for _ in range(max(n_steps // M - 1, 0))]
+        # N > 1: device + pinned buffers of the one exchange, a slot per reduction of a pass
+        exchange = sharding.MomentExchange(plan, n_slots=n_steps // M, backend=args.backend) if world > 1 else None
+        launches = {"n": 0}
+        ens_tilt = any(p["A"] != 0.0 for p in sets)
+        step_launches = (2 if ens_tilt else 1) * -(-M // (65536 if ens_tilt else 2**30))
+        # parameter records marshalled once (host side); abm_create copies them to the device
+        params = abm.make_params(sets, stream=stream.cuda_stream, snapshot_every=wl.snapshot_every,
+                                 traj_base=plan.traj_base, traj_set_stride=plan.traj_set_stride)
+        params_bytes = len(sets) * abm.C.sizeof(abm.abm_params)
+
+        def one_pass(e2e, ev=None):
+            """The whole hot path once.  Returns the moments (host)."""
+            with torch.cuda.stream(stream):
+                ens = abm.Ensemble(params, n_particles, wl.seed, stream=stream)    # S0 (1 kernel)
+                launches["n"] += 1
+                if wl.snapshot_every:
+                    ens.bind_snapshot()                                            # S5 (1 kernel)
+                    launches["n"] += 1
+                m = None
+                for j in range(n_steps // M):
+                    if ev is not None:
+                        ev[j][0].record(stream)
+                    ens.step(M)                                                    # S1-S5, S7
+                    if ev is not None:
+                        ev[j][1].record(stream)
+                    launches["n"] += step_launches
+                    if world > 1:                          # S6 (2 kernels) + all-reduce, enqueued: no host round trip
+                        exchange.enqueue(ens, j)
+                    elif j + 1 < n_steps // M:     # intermediate reductions: enqueued, no host round trip
+                        ens.moments_async(mom_slots[j][0])                         # S6 (2 kernels)
+                    else:                          # the last one waits: every record is on the host now
+                        m = ens.moments(mom_out)                                   # S6 (2 kernels)
+                    launches["n"] += 2
+                if e2e:
+                    abm.abm_snapshot_host(ens.ctx, host_frame.numpy(), frame_cols * frame_item)
+                    launches["n"] += 1
+                ens.close()                                # waits for the stream: every record is on the host
+                if world > 1:
+                    m = exchange.result(n_steps // M - 1)
+            return m
+
+        for _ in range(max(warmup, 0)):
+            one_pass(False)
+            one_pass(True)
+        barrier()
+
+        # ---- device-timed arm -------------------------------------------------------------------
+        ev_pass = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                   for _ in range(steps)]
+        ev_kern = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                    for _ in range(n_steps // M)] for _ in range(steps)]   # around every abm_step
+        launches["n"] = 0
+        barrier()
+        wall0 = time.perf_counter()
+        with ClockSampler(torch.cuda.current_device()) as clk:
+            for i in range(steps):
+                flush.fill_(i & 0xff)                       # L2 flush between timed iterations
+                torch.cuda.synchronize()
+                ev_pass[i][0].record(stream)
+                m = one_pass(False, ev_kern[i])
+                ev_pass[i][1].record(stream)
+            barrier()
+        wall = time.perf_counter() - wall0
+        gpu_launches = launches["n"]
+        t_pass_ms = [a.elapsed_time(b) for a, b in ev_pass]
+        t_dev = sum(t_pass_ms) * 1e-3
+        t_kern_ms = [sum(a.elapsed_time(b) for a, b in evs) for evs in ev_kern]   # per pass, all abm_step calls
+
+        # ---- end-to-end arm (host params -> host frame + moments), wall clock ---------------------
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(steps):
+            one_pass(True)
+        barrier()
+        t_e2e = time.perf_counter() - t0
+
+        # ---- the paper's "offset time" (PAPER.md:122): 20 launches of one step, the last 15 (PAPER.md:100) ----
+        t_off = None
+        if with_offset:
+            with torch.cuda.stream(stream):
+                ens = abm.Ensemble(params, n_particles, wl.seed, stream=stream)
+                if wl.snapshot_every:
+                    ens.bind_snapshot()
+                ev_off = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                          for _ in range(20)]
+                for a, b in ev_off:
+                    a.record(stream)
+                    ens.step(1)
+                    b.record(stream)
+                stream.synchronize()
+                ens.close()
+            t_off = [a.elapsed_time(b) for a, b in ev_off][5:]
+
+        tt = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=coll_dev)
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_dev, t_e2e = float(tt[0]), float(tt[1])
+
+        # particle-steps of the whole job: weak = `world` copies of the workload, strong = the one workload
+        psteps_rank = T * n_steps
+        psteps_job = wl.particle_steps * (world if args.scaling == "weak" else 1) * steps
+        value = psteps_job / t_dev
+        clocks = clk.summary()
+
+        out = {
+            "metric": "particle-steps/sec", "value": value, "unit": "particle-steps/s",
+            "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": 1e3 * t_dev / steps, "higher_is_better": True, "scaling": args.scaling,
+            "ms_per_step_sd": statistics.pstdev(t_pass_ms) if len(t_pass_ms) > 1 else None,   # this rank's passes
+            "offset_ms": {"mean": statistics.mean(t_off), "sd": statistics.pstdev(t_off),
+                          "protocol": "20 launches of 1 step, last 15 (PAPER.md:100, :122)"} if t_off else None,
+            "vs_baseline": None,   # BASELINE.md: the paper states no throughput for this path
+            "dtype": "f64" if fp64 else "f32", "data": "synthetic",
+            "config": {"workload": wl.name, "baseline_config": cfg_id, "trajectories_per_gpu": T,
+                       "param_sets": wl.n_param_sets, "sim_steps": n_steps,
+                       "snapshot_every": wl.snapshot_every, "moments_every": M,
+                       "integrator": "heun" if sets[0]["integrator"] else "euler-maruyama", "rng": args.rng,
+                       "scaling": args.scaling, "shard": plan.split if world > 1 else "none",
+                       "l2": "flushed between timed iterations (256 MiB fill)",
+                       "pass": "create+init, bind frame, integrate, moments, destroy"},
+            "e2e": {"value": psteps_job / t_e2e, "unit": "particle-steps/s",
+                    "h2d_bytes_per_step": int(params_bytes),
+                    "d2h_bytes_per_step": int(host_frame.numel() * host_frame.element_size()
+                                              + 80 * len(sets) * (n_steps // M)),
+                    "timer": "wall clock, host parameter records -> pinned host frame + moments"},
+            "gpu_launches": gpu_launches,
+            "clocks": clocks,
+            "wall_s_timed_region": wall,
         }
+        if t_kern_ms:
+            t_k = statistics.mean(t_kern_ms) * 1e-3
+            lane_instr = I_ALG[cfg_id] * psteps_rank
+            lanes = LANES_FP64 if fp64 else LANES_PER_SM
+            peak = N_SM * lanes * f_max
+            achieved = lane_instr / t_k
+            sm_mhz = clocks.get("sm_mhz") or (f_max / 1e6)
+            cap, cap_src = ncu_capture(cfg_id) if (not args.sim_steps and args.rng == "philox" and world == 1) else \
+                (None, "no capture of this launch (--sim-steps / --rng xorshift / sharded)")
+            philox = args.rng == "philox"
+            out["roofline"] = {
+                "bound": "alu",
+                "kernel": "abm::step_kernel_small" if (not fp64 and args.rng == "philox" and
+                                                        T <= 96 * torch.cuda.get_device_properties(0).multi_processor_count)
+                else "abm::step_kernel",   # AUTO: up to three 32-trajectory CTAs per SM (include/abm.h)
+                "achieved": achieved / 1e12 if philox else None,
+                "peak": peak / 1e12,
+                "unit": "Tinstr/s (FP64-pipe lane operations)" if fp64 else "Tinstr/s (warp-lane instructions)",
+                "frac": achieved / peak if philox else None,     # I_alg is frozen for the Philox path only
+                "frac_at_sustained_clock": achieved / (N_SM * lanes * sm_mhz * 1e6) if philox else None,
+                "i_alg_per_particle_step": I_ALG[cfg_id] if philox else None,
+                # the same with what the kernel executes per particle-step in place of I_alg (ncu capture): how busy
+                # the issue slots (fp64: the FP64 pipe) are, whatever the instructions are worth
+                "frac_executed": cap["executed"] * psteps_rank / t_k / peak if cap else None,
+                "executed_per_particle_step": cap["executed"] if cap else None,
+                "particle_steps_per_pass": psteps_rank,
+                "kernel_ms": 1e3 * t_k, "kernel_ms_sd": statistics.pstdev(t_kern_ms) if len(t_kern_ms) > 1 else None,
+                "kernel_launches_per_pass": step_launches * (n_steps // M),
+                "kernel_share_of_pass": sum(t_kern_ms) / sum(t_pass_ms),
+                "peak_source": f"148 SMs x {lanes} lanes x sm_max_mhz {f_max / 1e6:.0f} MHz, {peak_src}",
+                "traffic": cap["traffic"] if cap else None, "traffic_source": cap_src,
+                "hbm_algorithmic_bytes_per_launch": int(T * (24 + 8 * (n_steps // wl.snapshot_every
+                                                                       if wl.snapshot_every else 0))),
+            }
+        return out, m
+
+    out, m = measure(wl, cfg_id, args.steps, args.warmup)
+    # The other BASELINE.json configs, measured AFTER the headline's timed regions (which they cannot disturb) with
+    # the same protocol and fewer passes, so that the one line the driver runs carries all five (SURVEY.md 8(d)).
+    if world == 1 and args.all_configs and cfg_id == 1 and not args.sim_steps and args.rng == "philox":
+        extra = {}
+        for other in (0, 2, 3, 4):
+            o, _ = measure(W.CONFIGS[other](), other, args.all_configs, 1, with_offset=False)
+            r = o["roofline"]
+            extra[o["config"]["workload"]] = {
+                "value": o["value"], "ms_per_step": o["ms_per_step"], "steps": o["steps"], "dtype": o["dtype"],
+                "kernel": r["kernel"], "kernel_ms": r["kernel_ms"], "kernel_ms_sd": r["kernel_ms_sd"],
+                "frac": r["frac"], "frac_executed": r["frac_executed"], "unit": r["unit"],
+                "e2e": o["e2e"]["value"], "clocks": o["clocks"]}
+        out["all_configs"] = extra
     if rank == 0:
         if world == 1 and not args.no_cpu_baseline:
             out["cpu_baseline"] = cpu_baseline(wl)
@@ -476,6 +513,12 @@ def main():
     ap.add_argument("--rng", default="philox", choices=["philox", "xorshift"],
                     help="generator A/B (SURVEY.md 8(f) NEXT-4); the headline and the roofline are Philox")
     ap.add_argument("--sim-steps", type=int, default=0, help="override the config's step count")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: every rank a full copy on its own trajectory indices (weak, default), or the one "
+                         "ensemble divided over the ranks (strong: [gT/G, (g+1)T/G), SURVEY.md 8(e))")
+    ap.add_argument("--all-configs", type=int, default=3, metavar="PASSES",
+                    help="after the headline (config 1, N = 1) also time configs 0, 2, 3, 4 with this many passes "
+                         "each -> \"all_configs\" in the line; 0 = skip")
     args = ap.parse_args()
     wl = W.CONFIGS[args.config]()
     if args.sim_steps:

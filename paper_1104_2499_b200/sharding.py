@@ -16,7 +16,7 @@ or, without any host round trip between the reduction kernel and the collective 
     ex = MomentExchange(plan, n_slots=20)                           # device + pinned host buffers
     for j in range(20):
         ens.step(1000); ex.enqueue(ens, j)                          # reduction, all-reduce, async copy: no wait
-    torch.cuda.current_stream().synchronize()
+    ens.stream.synchronize()
     m = [ex.result(j) for j in range(20)]
 """
 from dataclasses import dataclass
@@ -113,41 +113,51 @@ class MomentExchange:
     """The exchange of the sharded path kept on the device: `abm_moment_sums_dev` writes this
     rank's raw sums into its rows of a [n_sets_total, 8] float64 CUDA tensor, one `all_reduce` (NCCL over
     NVLink) sums the tensor in place across ranks, and an asynchronous copy brings it to pinned host memory --
-    all enqueued on the current stream, nothing waits, so moments every M steps do not stall the integration.
+    nothing waits, so moments every M steps do not stall the integration.
     `result(slot)` finalises on the host (`abm_moments_from_sums`) after the caller has synchronised.
 
+    Stream order: the library enqueues the reduction on the ensemble's stream (`ens.stream`, the one its context
+    was created with), so `enqueue` issues every torch operation -- the zero fill, the collective, the copy to
+    the host -- on THAT stream as well, whatever torch's current stream is at the call.  The buffers are
+    zero-filled at construction on the then-current stream, which the constructor waits for.  Synchronise
+    `ens.stream` before `result`.
+
     backend gloo (rehearsal with ranks sharing one GPU; gloo reduces host tensors): the sums take a synchronous
-    detour through the host, everything else is the same code.  world == 1 skips the collective.
+    detour through the host, everything else is the same code.  world == 1 skips the collective unless
+    `always_collective` is set (a one-rank NCCL group is legal and exercises the very calls of the N-rank job).
     """
 
-    def __init__(self, plan: ShardPlan, n_slots: int = 1, group=None, backend: str = "nccl"):
+    def __init__(self, plan: ShardPlan, n_slots: int = 1, group=None, backend: str = "nccl",
+                 always_collective: bool = False):
         import torch
         self._torch, self.plan, self.group, self.backend = torch, plan, group, backend
+        self.collective = plan.world > 1 or always_collective
         shape = (n_slots, plan.n_sets_total, 8)
         self.dev = torch.zeros(shape, dtype=torch.float64, device="cuda")
         self.host = torch.zeros(shape, dtype=torch.float64, pin_memory=True)
+        torch.cuda.current_stream().synchronize()   # the fills are done before any other stream touches the buffers
         self.steps = [0] * n_slots
 
     def enqueue(self, ens, slot: int):
         torch, plan = self._torch, self.plan
         buf = self.dev[slot]
-        if plan.split == "sets" and plan.world > 1:
-            buf.zero_()                           # rows of the other ranks' sets: filled by the all-reduce
-        rows = buf[plan.set_first:plan.set_first + plan.n_sets]
-        ens.moment_sums_dev(rows)
-        self.steps[slot] = ens.step_count
-        if plan.world > 1:
-            import torch.distributed as dist
-            if self.backend == "nccl":
-                dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=self.group)
-            else:
-                t = buf.cpu()
-                dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
-                buf.copy_(t)
-        self.host[slot].copy_(buf, non_blocking=True)
+        with torch.cuda.stream(ens.stream):        # the stream abm_moment_sums_dev enqueues on
+            if plan.split == "sets" and self.collective:
+                buf.zero_()                       # rows of the other ranks' sets: filled by the all-reduce
+            rows = buf[plan.set_first:plan.set_first + plan.n_sets]
+            ens.moment_sums_dev(rows)
+            self.steps[slot] = ens.step_count
+            if self.collective:
+                import torch.distributed as dist
+                if self.backend == "nccl":
+                    dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=self.group)
+                else:
+                    t = buf.cpu()
+                    dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
+                    buf.copy_(t)
+            self.host[slot].copy_(buf, non_blocking=True)
 
     def result(self, slot: int):
-        """Finalised moments of the whole job (valid once the stream the calls were enqueued on has been
-        synchronised)."""
+        """Finalised moments of the whole job (valid once the ensemble's stream has been synchronised)."""
         from . import binding
         return binding.abm_moments_from_sums(self.host[slot].numpy(), self.steps[slot])

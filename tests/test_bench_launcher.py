@@ -47,6 +47,27 @@ def test_bare_gpus_flag_runs_two_ranks_gloo_rehearsal():
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("config,shard", [("3", "particles"), ("2", "sets")])
+def test_strong_scaling_arm_two_ranks_gloo_rehearsal(config, shard):
+    """--scaling strong divides the ONE ensemble: realisations of the single set (config[3]) or whole parameter
+    sets (config[2]) per rank; the job's particle-steps are those of the undivided workload, and the exchanged
+    moments count all of its trajectories."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--backend", "gloo",
+                        "--scaling", "strong", "--config", config, "--sim-steps", "1000", "--steps", "2",
+                        "--warmup", "1"], capture_output=True, text=True, env=env, timeout=900)
+    assert r.returncode == 0, r.stderr[-3000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["scaling"] == "strong" and out["config"]["shard"] == shard
+    total = {"3": 1_048_576, "2": 4_194_304}[config]
+    assert out["config"]["trajectories_per_gpu"] == total // 2
+    assert abs(out["value"] * out["ms_per_step"] * 1e-3 - total * 1000) < 1e-6 * total * 1000
+    assert out["result"]["step"] == 1000
+
+
+@pytest.mark.gpu
 def test_gpus_flag_must_match_world_size():
     env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--config", "0"],

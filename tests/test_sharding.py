@@ -200,3 +200,92 @@ def test_two_ranks_device_side_exchange_equals_one_context(name):
             assert np.array_equal(got["n"], want["n"]) and np.array_equal(got["step"], want["step"])
             for k in ("mean_x", "var_x", "mean_v", "var_v", "mean_e", "mean_dx", "mean_dx2", "mean_x2"):
                 assert np.allclose(got[k], want[k], rtol=1e-12, atol=1e-13), (name, j, k)
+
+
+# ---- MomentExchange on a stream that is not torch's current one ---------------------------
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("scaling", ["weak", "strong"])
+def test_exchange_is_ordered_on_the_ensembles_own_stream(scaling):
+    """The context enqueues its reduction on the stream it was created with; MomentExchange must put its own
+    torch operations (zero fill, copy to the host) on that same stream even when the caller's current stream is
+    another one.  The default stream is kept busy meanwhile, so work wrongly issued there would run late."""
+    import torch
+    from paper_1104_2499_b200 import binding as abm
+    wl = W.config2()
+    sets = [wl.set_params(s) for s in range(0, wl.n_param_sets, wl.n_param_sets // 37)]
+    chunks = [40, 24, 36, 8]
+    side = torch.cuda.Stream()
+    plan = sharding.shard_plan(200, len(sets), 0, 1, scaling)
+    ex = sharding.MomentExchange(plan, n_slots=len(chunks), always_collective=False)
+    ballast = torch.empty(1 << 28, dtype=torch.float32, device="cuda")     # 1 GiB fills on the default stream
+    with abm.Ensemble(sets, 200, wl.seed, stream=side) as ens:
+        assert torch.cuda.current_stream() != side
+        for j, n in enumerate(chunks):
+            ballast.fill_(float(j))
+            ens.step(n)
+            ex.enqueue(ens, j)                                             # called OUTSIDE any stream block
+        ens.stream.synchronize()
+        got = [ex.result(j) for j in range(len(chunks))]
+    torch.cuda.synchronize()
+    with abm.Ensemble(sets, 200, wl.seed) as twin:                          # same trajectories, waiting calls
+        for j, n in enumerate(chunks):
+            twin.step(n)
+            assert got[j].tobytes() == twin.moments().tobytes(), j
+
+
+# ---- the NCCL calls of the N-rank job, executed with a one-rank group on the box's one GPU -------------
+
+def _nccl_one_rank_main(port, q):
+    import torch
+    import torch.distributed as dist
+    from paper_1104_2499_b200 import binding as abm
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    torch.cuda.set_device(0)
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+    try:
+        wl = W.config2()
+        sets = [wl.set_params(s) for s in range(0, wl.n_param_sets, wl.n_param_sets // 19)]
+        chunks = [20, 12, 40]
+        out = {}
+        for scaling in ("weak", "strong"):                                # "replica" and "sets" splits
+            plan = sharding.shard_plan(128, len(sets), 0, 1, scaling)
+            ex = sharding.MomentExchange(plan, n_slots=len(chunks), backend="nccl", always_collective=True)
+            side = torch.cuda.Stream()
+            with abm.Ensemble(sets, 128, wl.seed, stream=side) as ens:
+                for j, n in enumerate(chunks):
+                    ens.step(n)
+                    ex.enqueue(ens, j)                                     # abm_moment_sums_dev -> ncclAllReduce -> D2H
+                ens.stream.synchronize()
+                got = [ex.result(j).tobytes() for j in range(len(chunks))]
+            with abm.Ensemble(sets, 128, wl.seed) as twin:
+                want = []
+                for n in chunks:
+                    twin.step(n)
+                    want.append(twin.moments().tobytes())
+            out[scaling] = (got == want)
+        q.put(("ok", out, dist.get_backend(), dist.get_world_size()))
+    except Exception as exc:                                               # report instead of hanging the parent
+        q.put(("error", repr(exc), None, None))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_nccl_branch_runs_with_a_one_rank_group():
+    """`dist.init_process_group("nccl", device_id=...)` and the in-place all-reduce of the CUDA tensor between
+    `abm_step` calls -- the branch bench.py takes under torchrun -- executed for real: a one-rank NCCL
+    communicator on cuda:0.  The sum over one rank is the identity, so the moments equal abm_moments bit for bit."""
+    import torch
+    import torch.multiprocessing as mp
+    assert torch.cuda.is_available()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    p = ctx.Process(target=_nccl_one_rank_main, args=(_free_port(), q))
+    p.start()
+    status, out, backend, world = q.get(timeout=300)
+    p.join(60)
+    assert status == "ok", out
+    assert p.exitcode == 0
+    assert backend == "nccl" and world == 1
+    assert out == {"weak": True, "strong": True}
