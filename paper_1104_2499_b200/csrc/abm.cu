@@ -98,7 +98,7 @@ Coef<Real> make_coef(const abm_params& p) {
   if (sizeof(Real) == 4) {
     c.th_s = static_cast<Real>(g);                      // radians
     c.th_o = static_cast<Real>(g * p.phi);
-    c.s2 = static_cast<Real>(-2.0 * (2.0 * p.D * p.dt) * 0.6931471805599453094);  // -2 sigma^2 ln2
+    c.s2 = static_cast<Real>(2.0 * (2.0 * p.D * p.dt));  // 2 sigma^2
   } else {
     c.th_s = static_cast<Real>(2.0 / p.L);              // half-turns (cospi)
     c.th_o = static_cast<Real>(2.0 * p.phi / p.L);

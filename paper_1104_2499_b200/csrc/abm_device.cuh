@@ -189,7 +189,7 @@ struct Coef {
   Real gamma0, d, q, c;
   Real k0, k1, k2;     // -U'(x) + F0 = k0 + k1 cos(th) + k2 cos(th)^2
   Real th_s, th_o;     // fp32: th = th_s x + th_o [rad];  fp64: th/pi = th_s x + th_o
-  Real s2;             // fp32: -2 sigma^2 ln 2 (so sigma^2 (-2 ln u) = s2 lg2 u); fp64: sigma
+  Real s2;             // fp32: 2 sigma^2 (so rho^2 = s2 lambda, lambda = -ln u1, see box_muller_f32); fp64: sigma
   Real A;              // tilt amplitude
   Real L, v0, e0, sv;  // init: x0 = L u, v0, e0, sv = sqrt(D/gamma0)
   Real bm_o;           // fp32: 2 pi 2^-24 - 3 pi, offset of the Box-Muller angle (see S2)
@@ -230,11 +230,29 @@ __device__ __forceinline__ float uniform_f32(uint32_t w) {
   return __fadd_rn(m, -(1.0f - 0x1p-24f));  // exact
 }
 
+// The radius.  lg2.approx is accurate to 2^-22 ABSOLUTELY on (1/2, 2), so as u1 -> 1, where the logarithm goes to
+// 0, its relative error -- hence that of rho -- grows without bound: 63 % at u1 = 1 - 2^-24, i.e. 2.2e-4 sigma on
+// v.  The exhaustive 100-step comparison with the oracle (every trajectory of configs [1-3]) found exactly these
+// draws: 3 + 2 trajectories beyond 1e-5 in configs [2], [3], each with a uniform within 10^-6 of 1.  Branch-free
+// repair, three instructions per pair (a branch anywhere inside the loop trip cuts the basic block in which ptxas
+// interleaves Philox rounds and floating-point work: measured +15 %; two blocks of look-ahead with the test at
+// the loop boundary: +8 %): with t = 1 - u1 (exact in fp32) and lambda = -ln u1 = t + t^2/2 + ... >= t,
+//     lam = max(-ln2 lg2.approx(u1) - B, t),    B = ln2 2^-22 (the error bound, so that the first term <= lambda),
+// is never above lambda + 0 and never below max(t, lambda - 2B): |lam - lambda| <= min(2B, t^2/2).  The radius
+// sqrt(2 lam) is then off by at most 8e-6 (at t = 8e-4, rho = 0.04) instead of 2.2e-4, by 2.7e-7 at rho = 1.2 --
+// 3.6e-7 on v at the largest sigma of the configs (D = 1) against a tolerance of 1e-5.
+constexpr float BM_LG2_BIAS = 0.6931471805599453f * 0x1p-22f;
+
 __device__ __forceinline__ Normal2f box_muller_f32(uint32_t wa, uint32_t wb, float s2,
                                                    float bm_o) {
   Normal2f o;
-  const float u1 = uniform_f32(wa);
-  o.rho = fast_sqrt(__fmul_rn(fast_lg2(u1), s2));
+  const float m1 = __uint_as_float((wa >> 9) + 0x3f800000u);
+  const float u1 = __fadd_rn(m1, -(1.0f - 0x1p-24f));   // uniform_f32(wa), exact
+  const float t = __fadd_rn(1.0f, -u1);                 // exact: (2^24 - 2k - 1) 2^-24 has 24 bits (2 - 2^-24 - m1 would
+                                                        // not be: 2 - 2^-24 is no fp32 number)
+  // lam <= -ln u1 whatever the sign of MUFU.LG2's error; t <= -ln u1 always: the larger of the two (see above)
+  const float lam = fmaxf(__fmaf_rn(fast_lg2(u1), -0.6931471805599453f, -BM_LG2_BIAS), t);
+  o.rho = fast_sqrt(__fmul_rn(lam, s2));
   // 2 pi u2 - pi = 2 pi (m - 1 + 2^-24) - pi = 2 pi m + bm_o,  bm_o = 2 pi 2^-24 - 3 pi
   const float m2 = __uint_as_float((wb >> 9) + 0x3f800000u);
   const float ang = __fmaf_rn(m2, 6.283185307179586f, bm_o);

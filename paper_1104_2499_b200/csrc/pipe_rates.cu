@@ -555,7 +555,7 @@ __device__ unsigned long long g_bm[6];  // bit patterns of non-negative doubles:
 __global__ void bm_accuracy_kernel() {
   const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;  // 23-bit uniform index
   const uint32_t w = k << 9;
-  const float s2 = static_cast<float>(-2.0 * 0.6931471805599453);   // sigma = 1
+  const float s2 = 2.0f;   // 2 sigma^2, sigma = 1
   const float bm_o = static_cast<float>(2.0 * 3.141592653589793 * 0x1p-24 - 3.0 * 3.141592653589793);
   const abm::Normal2f z = abm::box_muller_f32(w, w, s2, bm_o);
   const double u = (static_cast<double>(k) + 0.5) * 0x1p-23;

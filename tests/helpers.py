@@ -31,6 +31,46 @@ def oracle_states(oracle, params, seed, traj_idx, n_steps, step_first=0, state=N
     return out
 
 
+def oracle_states_all(oracle, sets, n_particles, seed, n_steps, threads=None):
+    """Oracle state (float64 [n_sets * n_particles, 3], local order k = set * n_particles + r) of EVERY trajectory
+    of an ensemble after n_steps steps from the init block.  One set: one call, split over the host threads
+    by trajectory range.  Many sets: a pool of host threads, each taking a contiguous range of sets and calling
+    the oracle once per set (single-threaded calls; ctypes drops the GIL).  No arithmetic here."""
+    import concurrent.futures as cf
+    threads = threads or oracle.host_threads()
+    n_sets = len(sets)
+    out = np.empty((n_sets * n_particles, 3), np.float64)
+    if n_sets == 1:
+        x, v, e = oracle.init_many(sets[0], seed, n_particles, 0)
+        oracle.run(sets[0], seed, x, v, e, 0, n_steps, 0, threads=threads)
+        out[:, 0], out[:, 1], out[:, 2] = x, v, e
+        return out
+
+    def work(s0, s1):
+        for s in range(s0, s1):
+            first = s * n_particles
+            x, v, e = oracle.init_many(sets[s], seed, n_particles, first)
+            oracle.run(sets[s], seed, x, v, e, 0, n_steps, first, threads=1)
+            blk = out[first:first + n_particles]
+            blk[:, 0], blk[:, 1], blk[:, 2] = x, v, e
+
+    bounds = np.linspace(0, n_sets, threads + 1).astype(int)
+    with cf.ThreadPoolExecutor(threads) as pool:
+        for f in [pool.submit(work, int(bounds[i]), int(bounds[i + 1])) for i in range(threads)]:
+            f.result()
+    return out
+
+
+def scale_rel_err_elements(got, want, n_sets=1):
+    """Reading G14 element by element: |got - want| / max(|want|, RMS of that variable over the ensemble the
+    trajectory belongs to -- the realisations of ITS parameter set).  Returns the [n, 3] array of errors."""
+    got, want = np.asarray(got, np.float64), np.asarray(want, np.float64)
+    w = want.reshape(n_sets, -1, 3)
+    rms = np.sqrt(np.mean(w * w, axis=1, keepdims=True))                     # [n_sets, 1, 3]
+    scale = np.maximum(np.abs(w), np.maximum(rms, 1e-300))
+    return (np.abs(got.reshape(n_sets, -1, 3) - w) / scale).reshape(-1, 3)
+
+
 def scale_rel_err(got, want):
     """Reading G14: per variable, |got - want| / max(|want|, RMS of that variable over
     the compared ensemble).  Returns the max over trajectories, per variable (x, v, e)."""
