@@ -57,7 +57,7 @@ N_SM, LANES_PER_SM = 148, 128
 # I_alg counts the ~60 DFMA-pipe operations per particle-step and its peak is 64 lanes.
 LANES_FP64 = 64
 # What the committed `ncu --set full` captures of the launches bench.py times say about the step kernel
-# (profiles/r02_step_kernels_ncu_full.md), per launch: dram__bytes_read.sum + dram__bytes_write.sum (`traffic`)
+# (profiles/r03_step_kernels_ncu_full.md), per launch: dram__bytes_read.sum + dram__bytes_write.sum (`traffic`)
 # and what the kernel EXECUTES per particle-step -- warp-lane instructions (smsp__inst_executed.sum x 32 / particle-
 # steps) for the fp32 kernels, FP64-pipe lane operations (smsp__inst_executed_pipe_fp64.sum x 32 / particle-steps)
 # for config[4] -- from which `roofline.frac_executed` follows: the fraction of the issue slots (or of the FP64
@@ -67,18 +67,19 @@ LANES_FP64 = 64
 # The frame (one, overwritten) and the state stay in the 126 MB L2 during a launch, so the traffic is far BELOW
 # the algorithmic bytes.  Every capture is of the full launch bench.py times (config[3]: one of the 20 launches of
 # 1,000 steps a pass is made of).
-_SRC = dict(kernels="0de9475028dab8808e94983a210a9710ec9535ff", device="06fe9e9ccfc6a44b54143a1038a941dd9225e44e",
-            summary="profiles/r02_step_kernels_ncu_full.md")
+_SRC = dict(kernels="0de9475028dab8808e94983a210a9710ec9535ff", device="41e835be8e554d8dda9c5a0b24acdd14995b1e13",
+            summary="profiles/r03_step_kernels_ncu_full.md")
 NCU_CAPTURE = {
     # cfg: dict(traffic=bytes per launch, executed=per particle-step, kernels=blob of csrc/abm_kernels.cuh,
     #           device=blob of csrc/abm_device.cuh, summary=file under profiles/)
-    0: dict(traffic=79_872, executed=39.23, **_SRC),
-    1: dict(traffic=12_652_032, executed=29.15, **_SRC),
-    2: dict(traffic=57_197_568, executed=28.54, **_SRC),
+    0: dict(traffic=80_128, executed=40.89, **_SRC),
+    1: dict(traffic=12_692_480, executed=30.78, **_SRC),
+    2: dict(traffic=56_665_600, executed=30.29, **_SRC),
     # one of the 20 launches (1,000 steps each) of a pass
-    3: dict(traffic=21_008_640, executed=48.86, **_SRC),
-    # FP64-pipe operations (146 per Philox block in the loop; ncu: sm__pipe_fp64_cycles_active 71.55 %)
-    4: dict(traffic=156_946_176, executed=36.5, **_SRC),
+    3: dict(traffic=21_009_408, executed=50.36, **_SRC),
+    # FP64-pipe operations (146 per Philox block in the loop; ncu: sm__pipe_fp64_cycles_active 71.55 %); the fp64
+    # kernel is the one of round 2 (same instruction count, 576.4 ms), so the operation count is carried over
+    4: dict(traffic=157_319_168, executed=36.5, **_SRC),
 }
 # Warp-lane instructions per particle-step of the xorshift variant are not frozen anywhere: no `frac` for it.
 
