@@ -67,7 +67,7 @@ LANES_FP64 = 64
 # The frame (one, overwritten) and the state stay in the 126 MB L2 during a launch, so the traffic is far BELOW
 # the algorithmic bytes.  Every capture is of the full launch bench.py times (config[3]: one of the 20 launches of
 # 1,000 steps a pass is made of).
-_SRC = dict(kernels="0de9475028dab8808e94983a210a9710ec9535ff", device="41e835be8e554d8dda9c5a0b24acdd14995b1e13",
+_SRC = dict(kernels="846dcb59299abdf7283dcc81d6fbb01e7b906435", device="41e835be8e554d8dda9c5a0b24acdd14995b1e13",
             summary="profiles/r03_step_kernels_ncu_full.md")
 NCU_CAPTURE = {
     # cfg: dict(traffic=bytes per launch, executed=per particle-step, kernels=blob of csrc/abm_kernels.cuh,

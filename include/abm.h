@@ -97,7 +97,10 @@ enum { ABM_INIT_V_CONST = 0, ABM_INIT_V_THERMAL = 1 }; /* abm_params.init_v */
  * a trajectory near a barrier top amplifies ANY fp32 rounding by exp(sqrt(max U'') t)).  Beyond that no
  * fp32 arithmetic meets 1e-5 after 100 steps: use ABM_FP64 or a smaller dt.  abm_get_accuracy reports
  * the mode in effect and whether the ensemble is beyond these limits.
- * Ignored in fp64.  Both modes consume the same random stream. */
+ * Ignored in fp64.  Both modes consume the same random stream.
+ * fp64 runs read two small Box-Muller tables that the library computes on the HOST in long double at first use: on
+ * one host results are bit-identical from run to run; between hosts of different architecture or libm an entry may
+ * differ in its last bit, so fp64 trajectories then agree to ~1e-16, not bit for bit. */
 enum { ABM_ACCURACY_AUTO = 0, ABM_ACCURACY_FAST = 1, ABM_ACCURACY_PRECISE = 2 };
 /* flag OR-ed into the value abm_get_accuracy returns: some set is stiffer than the mode in effect is
  * good for (FAST: S > 0.15, PRECISE: S > 0.3), so the fp32 state may deviate from an fp64 integration
@@ -119,7 +122,7 @@ enum { ABM_RNG_PHILOX = 0, ABM_RNG_XORSHIFT128 = 1 };
  *   AUTO         the library chooses by ensemble size.
  *   PER_THREAD   always one trajectory per thread (step_kernel).
  *   SPLIT_WARPS  the warp-specialised kernel (noise warps + integrating warps) wherever it applies
- *                (fp32, Philox, launches of whole Philox blocks), whatever the ensemble size. */
+ *                (fp32, Philox, launches of whole Philox blocks, up to (2^31 - 1) * 32 trajectories: its grid). */
 enum { ABM_STEP_KERNEL_AUTO = 0, ABM_STEP_KERNEL_PER_THREAD = 1, ABM_STEP_KERNEL_SPLIT_WARPS = 2 };
 
 typedef struct abm_ctx abm_ctx; /* opaque, owned by the library */
@@ -313,7 +316,8 @@ int abm_trim(void);
  * block's words instead of integrating with them -- the per-trajectory half of rounds 0-1 done once,
  * the per-block half fetched from the double-buffered shared-memory table that is refilled every 128
  * blocks, rounds 2-9 with the round keys the host computes, the look-ahead pipeline, and
- *   loop_shape 0: two blocks per loop trip (the fp32 kernels), 1: one block per trip (the fp64 kernels);
+ *   loop_shape 0: the loop as the fp32 kernels instantiate it, 1: as the fp64 kernels do (both run two blocks per
+ *   loop trip since round 2; the value only selects the instantiation);
  *   frame_every_blocks != 0: the loop is cut into segments of that many blocks as by a frame period of
  *   4 * frame_every_blocks steps (odd segments exercise the loop's one-block prologue).
  * A trajectory range that straddles a multiple of 2^32 runs the loop's table-free branch, as in abm_step.

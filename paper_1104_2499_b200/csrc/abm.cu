@@ -330,7 +330,10 @@ void stage_release(int device, cudaStream_t stream) {
 }
 
 // The fp64 Box-Muller tables (abm_device.cuh, NoiseTables<double>), computed once per process in extended
-// precision (long double: 64-bit mantissa on x86-64, 113 on aarch64) and rounded to double.
+// precision (long double: 64-bit mantissa on x86-64, 113 on aarch64) and rounded to double.  An entry may
+// therefore differ in its last bit between host architectures / libm versions: fp64 trajectories are bit-identical
+// across runs and launch splits on one host, and agree to ~1e-16 (not bit for bit) between hosts of different kinds
+// (include/abm.h says so).
 const double2* host_noise_tables() {
   static const std::vector<double2>* tab = [] {
     auto* t = new std::vector<double2>(NOISE_TABLE_N);
@@ -636,10 +639,15 @@ int abm_create(const abm_params* params, uint64_t n_particles, uint32_t n_param_
   c->tilt_A = n_param_sets == 1 ? p0.A : 1.0;
   c->real_size = c->precision == ABM_FP32 ? 4 : 8;
   // which step kernel (abm_params.step_kernel; results do not depend on it)
-  int n_sm_small = 148;
-  cudaDeviceGetAttribute(&n_sm_small, cudaDevAttrMultiProcessorCount, c->device);
+  int n_sm_small = 0;
+  if (cudaDeviceGetAttribute(&n_sm_small, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || n_sm_small <= 0) {
+    cudaGetLastError();
+    delete c;
+    return ABM_ECUDA;
+  }
+  // SPLIT_WARPS forced: wherever its grid of 32-trajectory CTAs fits the 2^31 - 1 limit; beyond it step_kernel runs
   c->small_max_traj = p0.step_kernel == ABM_STEP_KERNEL_PER_THREAD    ? 0
-                      : p0.step_kernel == ABM_STEP_KERNEL_SPLIT_WARPS ? ~0ull
+                      : p0.step_kernel == ABM_STEP_KERNEL_SPLIT_WARPS ? static_cast<uint64_t>(0x7fffffffu) * SMALL_TRAJ
                       : static_cast<uint64_t>(n_sm_small) * ABM_SMALL_MAX_CTAS_PER_SM * SMALL_TRAJ;
   c->split_coefs = n_param_sets > 1 && flags.shape_differs.load() == 0;
   c->precise = false;

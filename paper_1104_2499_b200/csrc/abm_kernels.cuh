@@ -492,8 +492,8 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint32_
             const uint32_t rest = in_chunk - done;
             const uint32_t seg = rest < to_snap ? rest : static_cast<uint32_t>(to_snap);  // >= 1
             // fp32: two blocks per loop trip -- the look-ahead words alternate between two register
-            // sets, so no moves rotate them and the loop overhead is halved (fp64 is short of
-            // registers: one block per trip).
+            // sets, so no moves rotate them and the loop overhead is halved (fp64 too since round 2:
+            // ABM_UNROLL2_F64 = 1; the one-block branch below is compiled only with -DABM_UNROLL2_F64=0).
             if constexpr ((sizeof(Real) == 4 || ABM_UNROLL2_F64 != 0) && ABM_UNROLL2 != 0) {
               if (seg & 1u) {
                 const uint4 u = *tp++;
@@ -583,7 +583,7 @@ __device__ __forceinline__ void run_steps(const StepArgs<Real>& a, const uint32_
 #define ABM_PHILOX_TABLE 1
 #endif
 
-// fp64: every CTA copies the Box-Muller tables (17.9 KB) from global to shared memory once per launch.
+// fp64: every CTA copies the Box-Muller tables (1281 x 16 B = 20.5 KB) from global to shared memory once per launch.
 __device__ __forceinline__ NoiseTables<float> stage_noise_tables(const StepArgs<float>&) { return {}; }
 __device__ __forceinline__ NoiseTables<double> stage_noise_tables(const StepArgs<double>& a) {
   for (int i = threadIdx.x; i < NOISE_TABLE_N; i += STEP_BLOCK) s_noise[i] = a.noise_tables[i];

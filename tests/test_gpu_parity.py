@@ -265,7 +265,7 @@ def test_normals_after_long_launches(abm, torch, oracle, K, traj_base):
 
 @pytest.mark.parametrize("precision,rng", [(1, 0), (0, 1), (1, 1)], ids=["f64_philox", "f32_xorshift", "f64_xorshift"])
 def test_normals_after_long_launches_fp64_and_xorshift(abm, oracle, precision, rng):
-    """The same pin for the fp64 block loop (one block per trip) and for the xorshift fast path (its own
+    """The same pin for the fp64 instantiation of the block loop (two blocks per trip as well since round 2) and for the xorshift fast path (its own
     look-ahead loop), with a frame every 12 steps so that segments of three blocks alternate with tails."""
     dt = 2.0**-10
     p = dict(W.DEFAULTS, precision=precision, rng=rng, A1=0.0, A2=0.0, d=0.0, q=0.0, c=0.0,
